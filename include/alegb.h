@@ -1,0 +1,157 @@
+/* alegb.h — C ABI of the B200-native ALE Galerkin-Boltzmann nodal-DG + SARK4 stage library.
+ *
+ * What the library computes (citations: PAPER.md line + equation of arxiv/paper_2607_00199; readings Rn are listed
+ * in DESIGN.md):
+ *
+ *   F(q, t) = - c sum_d A^_d dq/dx_d + v_G . grad q + N~(q) + LIFT( Fscale ( -A_n^- [q] + max(v_n, 0) [q] ) )
+ *
+ * the ALE Galerkin-Boltzmann semi-discrete operator on the mesh moved to time t (eq. 9, L65 eq. 4,
+ * L81-84 eq. 7, L115 for the split N~ / Lambda), and the semi-analytic Runge-Kutta step
+ *
+ *   q_ni  = q_n e^{-Lambda c_i dt} + dt sum_{j<i} a~_ij F_nj ,      q_n+1 = q_n e^{-Lambda dt} + dt sum_j b~_j F_nj
+ *
+ * with Lambda = diag(0,..,0,1/tau,..,1/tau) and the geometry re-evaluated at every stage time (L152-154).
+ * Everything is fp64; index arrays are int32.  All arithmetic of the path runs in CUDA kernels (sm_100a); there is
+ * no CPU fallback: every entry point that computes returns ALEGB_CUDA_ERROR if no device is usable.
+ *
+ * Conventions
+ *   - every call returns 0 (ALEGB_OK) or a negative alegb_status; nothing throws or aborts across the ABI;
+ *     alegb_last_error(ctx) returns a text for the last failure on that context.
+ *   - "HOST" pointers are read (or written) synchronously during the call and never retained.
+ *   - "DEVICE" pointers are owned by the caller (e.g. torch tensors), must be 16-byte aligned and valid on the
+ *     context's device; the library never frees or retains them beyond the enqueued work.
+ *   - compute calls enqueue on the given stream (a cudaStream_t passed as void*, NULL = default stream) and do NOT
+ *     synchronise.  alegb_mesh_upload, alegb_get_* and alegb_destroy synchronise the device.
+ *   - field layout: q[K][Nf][Np] (element, field, node), node fastest.  Nf = 6 (2-D) or 10 (3-D), field order
+ *     2-D (a00,a10,a01,a11,a20,a02) = the paper's q1..q6 (L43-51);
+ *     3-D (a000; a100,a010,a001; a110,a101,a011; a200,a020,a002)   (reading R3).
+ *     Node order: lattice order of the Warp & Blend set (L75): index of vertex 2 fastest, then vertex 3, then 4.
+ *   - element order is the upload order; the library does not permute.
+ */
+#ifndef ALEGB_H
+#define ALEGB_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct alegb_ctx alegb_ctx; /* opaque; the library owns everything inside */
+
+typedef enum {
+  ALEGB_OK = 0,
+  ALEGB_INVALID_ARG = -1, /* NULL where data is required, bad dim/N/kind, misaligned device pointer */
+  ALEGB_BAD_MESH = -2,    /* non-positive Jacobian at t=0, unmatched face without a tag, face shared by >2 elements,
+                             periodic direction with fewer than 3 cells (reading S4) */
+  ALEGB_NOT_READY = -3,   /* compute call before mesh_upload / set_params */
+  ALEGB_UNSUPPORTED = -4, /* (dim, N) without a compiled kernel */
+  ALEGB_CUDA_ERROR = -5   /* any CUDA runtime failure, including "no device" */
+} alegb_status;
+
+/* mesh-motion laws evaluated on the device from the t=0 vertex coordinates (reading R9:
+ * closed-form positions x_v(t) = X0_v + disp(X0_v,t), velocities d/dt of it, at the VERTICES only).
+ *   NONE           params: none
+ *   SINES_PRODUCT  PAPER.md:L227-231 (eq. 15): every coordinate += A sin(2 pi t/T) prod_d sin(kappa_d X_d + phi_d)
+ *                  params = [A, T, kappa_1..dim, phi_1..dim]
+ *   SINES_CROSS    PAPER.md:L251-256 (eq. 19): x_d += A sin(2 pi t/T) prod_{o != d} sin(k X_o + p)
+ *                  params = [A, T, k, p]
+ *   PLUNGE_BLEND   PAPER.md:L284-286 (eqs. 20-21): x_axis += h0 sin(omega t) b(|X0 - centre|),
+ *                  b = 1 (rho<=r1), 1-(6u^5-15u^4+10u^3), u=(rho-r1)/(r2-r1), 0 (rho>=r2)
+ *                  params = [h0, omega, r1, r2, axis, centre_1..dim]
+ *   CARANGIFORM    PAPER.md:L339-365 (reading R13): lateral displacement along `axis`
+ *                  (a0+a1 x~+a2 x~^2) sin(k X - omega t) B(d_eff) S(t);
+ *                  params = [a0, a1, a2, k, omega, R_rigid, beta, T_ramp, axis, Bcut]
+ *   USER           positions/velocities supplied by alegb_set_motion_user (device arrays, constant in time)
+ */
+typedef enum {
+  ALEGB_MOTION_NONE = 0,
+  ALEGB_MOTION_SINES_PRODUCT = 1,
+  ALEGB_MOTION_SINES_CROSS = 2,
+  ALEGB_MOTION_PLUNGE_BLEND = 3,
+  ALEGB_MOTION_CARANGIFORM = 4,
+  ALEGB_MOTION_USER = 5
+} alegb_motion_kind;
+
+/* Create a context for simplices of dimension dim (2 or 3) and polynomial order N (1..ALEGB_MAX_N) on CUDA device
+ * `cuda_device`.  Builds the reference element on the host: Warp & Blend nodes (L75), D_r,D_s(,D_t) = M^-1 S and
+ * LIFT = M^-1 M^f (L94-103).  *out is NULL on failure. */
+int alegb_create(alegb_ctx** out, int dim, int N, int cuda_device);
+int alegb_destroy(alegb_ctx* ctx);
+
+/* Mesh upload (HOST pointers, copied).  Straight-sided, conforming, positively oriented simplices (L73).
+ *   X0[Nverts*dim]        vertex coordinates at t = 0
+ *   EToV[K*(dim+1)]       element-to-vertex table; local face numbering: 2-D f1=(v1,v2), f2=(v2,v3), f3=(v3,v1);
+ *                         3-D f1=(v1,v2,v3), f2=(v1,v2,v4), f3=(v2,v3,v4), f4=(v1,v3,v4)
+ *   vertex_equiv[Nverts]  periodic master id of each vertex, or NULL (no periodicity)
+ *   EToB[K*(dim+1)]       0 interior, 1 moving no-slip wall, 2 far field (reading R11), or NULL (no boundary)
+ *   pml_sigma[K*dim]      per-element, per-direction damping of the absorbing layer, 0 = not in the layer
+ *                         (reading R12), or NULL
+ * Builds EToE/EToF and the trace maps vmapM/vmapP (L75, L196) by vertex ids, uploads everything, allocates the
+ * step workspace.  Synchronises. */
+int alegb_mesh_upload(alegb_ctx* ctx, int64_t Nverts, const double* X0, int64_t K, const int32_t* EToV,
+                      const int32_t* vertex_equiv, const int8_t* EToB, const double* pml_sigma);
+
+/* RT (L30), tau (L30; +inf allowed: collisionless), q_inf[Nf] far-field state (HOST, or NULL if no far-field faces) */
+int alegb_set_params(alegb_ctx* ctx, double RT, double tau, const double* q_inf);
+
+/* Prescribed motion law (see alegb_motion_kind); params is a HOST array, copied. */
+int alegb_set_motion(alegb_ctx* ctx, int kind, const double* params, int nparams);
+/* kind USER: DEVICE arrays [Nverts*dim] of vertex positions and velocities, copied device-to-device on the
+ * default stream and used for every subsequent evaluation until the motion is set again. */
+int alegb_set_motion_user(alegb_ctx* ctx, const double* d_xv, const double* d_vv);
+
+/* F = L(q) + N~(q) at time t (no -Lambda q), DEVICE q, F [K][Nf][Np].  In PML elements the library's current
+ * auxiliary fields enter F (term - sum_d sigma_d q~^d). */
+int alegb_rhs(alegb_ctx* ctx, double t, const double* d_q, double* d_F, void* stream);
+/* Same, plus the right-hand side of the auxiliary fields: d_aux, d_Faux DEVICE [Kpml][dim][Nf][Np]
+ * (Kpml = alegb_pml_count; order = ascending element index).  d_aux == NULL uses the library's own state. */
+int alegb_rhs_pml(alegb_ctx* ctx, double t, const double* d_q, const double* d_aux, double* d_F, double* d_Faux,
+                  void* stream);
+
+/* nsteps SARK4 steps of size dt from t0, in place on DEVICE q.  The library's PML auxiliary state advances with it. */
+int alegb_step(alegb_ctx* ctx, double* d_q, double t0, double dt, int nsteps, void* stream);
+/* One step, returning the four stage states q(1), q(2), q(3), q_{n+1}: d_stages DEVICE [4][K][Nf][Np].  d_q is not
+ * modified; the PML auxiliary state is advanced exactly as alegb_step would. */
+int alegb_step_debug(alegb_ctx* ctx, const double* d_q, double t0, double dt, double* d_stages, void* stream);
+
+/* Geometry of the mesh moved to time t.  Any output may be NULL.  DEVICE arrays:
+ *   d_vgeo[K][dim*dim+1]   (d xi_a/d x_d, a-major: r_x r_y (r_z) s_x ...; then J)
+ *   d_sgeo[K][Nfaces][dim+2] (unit outward normal n_1..n_dim, sJ, Fscale = sJ/J)
+ *   d_xv[Nverts][dim], d_vv[Nverts][dim] */
+int alegb_geometry(alegb_ctx* ctx, double t, double* d_vgeo, double* d_sgeo, double* d_xv, double* d_vv,
+                   void* stream);
+
+/* PML auxiliary state: count of layer elements, their ids (HOST out), zeroing, device-to-device get/set. */
+int64_t alegb_pml_count(const alegb_ctx* ctx);
+int alegb_pml_elements(const alegb_ctx* ctx, int32_t* elems /* HOST [Kpml] */);
+int alegb_pml_reset(alegb_ctx* ctx, void* stream);
+int alegb_pml_get(alegb_ctx* ctx, double* d_aux, void* stream);
+int alegb_pml_set(alegb_ctx* ctx, const double* d_aux, void* stream);
+
+/* Introspection (HOST out, any pointer may be NULL): sizes, reference nodes r,s,t [Np], operators row-major
+ * Dr,Ds,Dt [Np*Np], LIFT [Np*(Nfaces*Nfp)], trace maps [K*Nfaces*Nfp] (flattened node index e*Np+n), nodal
+ * quadrature weights w[Np] = 1^T M, barycentric interpolation matrix lam[Np*(dim+1)] (L192). */
+int alegb_get_sizes(const alegb_ctx* ctx, int* dim, int* N, int* Np, int* Nfp, int* Nfaces, int* Nfields,
+                    int64_t* K, int64_t* Nverts);
+int alegb_get_operators(alegb_ctx* ctx, double* r, double* s, double* t3, double* Dr, double* Ds, double* Dt,
+                        double* LIFT, int32_t* vmapM, int32_t* vmapP);
+int alegb_get_reference(const alegb_ctx* ctx, double* w, double* lam, int32_t* fmask);
+/* SARK4 coefficients the library would use for gamma = -dt/tau (L144-148; reading R6): HOST out
+ * a[6] = (a10,a20,a21,a30,a31,a32), b[4]. */
+int alegb_sark_coefficients(double gamma, double* a, double* b);
+
+int64_t alegb_workspace_bytes(const alegb_ctx* ctx);
+const char* alegb_last_error(const alegb_ctx* ctx);
+/* number of kernel launches the library has enqueued on this context since creation */
+int64_t alegb_launch_count(const alegb_ctx* ctx);
+/* Synchronous convenience entry for host buffers (HOST q [K][Nf][Np], updated in place): copies q to the device,
+ * runs nsteps SARK4 steps, copies the result back, synchronises.  Used for end-to-end timing. */
+int alegb_step_host(alegb_ctx* ctx, double* h_q, double t0, double dt, int nsteps);
+
+#define ALEGB_MAX_N 5
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ALEGB_H */

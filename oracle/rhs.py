@@ -131,7 +131,13 @@ class Problem:
             val = -np.einsum("kfg,kmg->kfm", Am, dq) + np.maximum(vn, 0.0)[:, None, :] * dq.transpose(0, 2, 1)
             flux[:, :, f * Nfp:(f + 1) * Nfp] = fs[:, None, None] * val
             if want_abs:
-                bound = (np.sqrt(3.0) * c + np.abs(vn))[:, None, :] * (np.abs(qP) + np.abs(qM)).transpose(0, 2, 1)
+                # R15: the same sum with every term replaced by its absolute value, field coupling included.
+                # The jump [q] = q+ - q- is a single IEEE subtraction of inputs (bit-identical in any
+                # implementation), so it is the primitive term here; bounding it by |q+| + |q-| would hide
+                # flux errors of relative size |q|/|[q]| behind the tolerance.
+                adq = np.abs(dq)                                # [K, Nfp, Nf]
+                bound = (np.einsum("kfg,kmg->kfm", np.abs(Am), adq)
+                         + np.maximum(vn, 0.0)[:, None, :] * adq.transpose(0, 2, 1))
                 flux_abs[:, :, f * Nfp:(f + 1) * Nfp] = fs[:, None, None] * bound
             if pml:
                 absA = An - 2.0 * Am                            # |A_n|

@@ -1,0 +1,235 @@
+"""Thin ctypes binding of the C-ABI library (include/alegb.h): argument marshalling only.
+
+Every function has the name of the C entry point it calls.  Device arrays are passed as torch CUDA tensors (their
+``data_ptr()`` is handed to the library) or as raw integer device addresses; host arrays as numpy arrays.  Nothing
+here computes: if libalegb.so is missing or fails to load, importing this module raises.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libalegb.so")
+
+OK, INVALID_ARG, BAD_MESH, NOT_READY, UNSUPPORTED, CUDA_ERROR = 0, -1, -2, -3, -4, -5
+MOTION_NONE, MOTION_SINES_PRODUCT, MOTION_SINES_CROSS, MOTION_PLUNGE_BLEND, MOTION_CARANGIFORM, MOTION_USER = range(6)
+STATUS_NAMES = {0: "OK", -1: "INVALID_ARG", -2: "BAD_MESH", -3: "NOT_READY", -4: "UNSUPPORTED", -5: "CUDA_ERROR"}
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError("libalegb.so is not built (run `python -m paper_2607_00199_b200.build`); "
+                      "the library has no fallback path")
+_lib = ctypes.CDLL(LIB_PATH)
+
+_c = ctypes
+_P = _c.c_void_p
+_SIGNATURES = {
+    "alegb_create": (_c.c_int, [_c.POINTER(_P), _c.c_int, _c.c_int, _c.c_int]),
+    "alegb_destroy": (_c.c_int, [_P]),
+    "alegb_mesh_upload": (_c.c_int, [_P, _c.c_int64, _P, _c.c_int64, _P, _P, _P, _P]),
+    "alegb_set_params": (_c.c_int, [_P, _c.c_double, _c.c_double, _P]),
+    "alegb_set_motion": (_c.c_int, [_P, _c.c_int, _P, _c.c_int]),
+    "alegb_set_motion_user": (_c.c_int, [_P, _P, _P]),
+    "alegb_rhs": (_c.c_int, [_P, _c.c_double, _P, _P, _P]),
+    "alegb_rhs_pml": (_c.c_int, [_P, _c.c_double, _P, _P, _P, _P, _P]),
+    "alegb_step": (_c.c_int, [_P, _P, _c.c_double, _c.c_double, _c.c_int, _P]),
+    "alegb_step_debug": (_c.c_int, [_P, _P, _c.c_double, _c.c_double, _P, _P]),
+    "alegb_step_host": (_c.c_int, [_P, _P, _c.c_double, _c.c_double, _c.c_int]),
+    "alegb_geometry": (_c.c_int, [_P, _c.c_double, _P, _P, _P, _P, _P]),
+    "alegb_pml_count": (_c.c_int64, [_P]),
+    "alegb_pml_elements": (_c.c_int, [_P, _P]),
+    "alegb_pml_reset": (_c.c_int, [_P, _P]),
+    "alegb_pml_get": (_c.c_int, [_P, _P, _P]),
+    "alegb_pml_set": (_c.c_int, [_P, _P, _P]),
+    "alegb_get_sizes": (_c.c_int, [_P] + [_c.POINTER(_c.c_int)] * 6 + [_c.POINTER(_c.c_int64)] * 2),
+    "alegb_get_operators": (_c.c_int, [_P] * 10),
+    "alegb_get_reference": (_c.c_int, [_P, _P, _P, _P]),
+    "alegb_sark_coefficients": (_c.c_int, [_c.c_double, _P, _P]),
+    "alegb_workspace_bytes": (_c.c_int64, [_P]),
+    "alegb_last_error": (_c.c_char_p, [_P]),
+    "alegb_launch_count": (_c.c_int64, [_P]),
+}
+for _name, (_res, _args) in _SIGNATURES.items():
+    _fn = getattr(_lib, _name)          # AttributeError here = the library does not export a declared symbol
+    _fn.restype, _fn.argtypes = _res, _args
+EXPORTED = sorted(_SIGNATURES)
+
+
+class AlegbError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__("%s: %s" % (STATUS_NAMES.get(status, status), message))
+        self.status = status
+
+
+def _dev(x):
+    """Device address of a torch CUDA tensor / raw int / None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if not x.is_cuda or not x.is_contiguous():
+        raise ValueError("device arrays must be contiguous CUDA tensors")
+    return x.data_ptr()
+
+
+def _host(x, dtype):
+    if x is None:
+        return None, None
+    a = np.ascontiguousarray(x, dtype=dtype)
+    return a, a.ctypes.data
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return stream if isinstance(stream, int) else stream.cuda_stream
+
+
+class Context:
+    """Owns one ``alegb_ctx``.  Methods are the C entry points without the ``alegb_`` prefix handling errors."""
+
+    def __init__(self, dim, N, cuda_device=0):
+        h = _P()
+        rc = _lib.alegb_create(ctypes.byref(h), dim, N, cuda_device)
+        if rc != OK:
+            raise AlegbError(rc, "alegb_create(dim=%d, N=%d, device=%d) failed" % (dim, N, cuda_device))
+        self._h = h
+        self.device = cuda_device
+        self.dim, self.N, self.Np, self.Nfp, self.Nfaces, self.Nf, self.K, self.Nverts = self.alegb_get_sizes()
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.alegb_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc != OK:
+            raise AlegbError(rc, (_lib.alegb_last_error(self._h) or b"").decode())
+
+    # ---- setup
+    def alegb_mesh_upload(self, X0, EToV, vertex_equiv=None, EToB=None, pml_sigma=None):
+        X0a, X0p = _host(X0, np.float64)
+        Ea, Ep = _host(EToV, np.int32)
+        va, vp = _host(vertex_equiv, np.int32)
+        ba, bp = _host(EToB, np.int8)
+        sa, sp = _host(pml_sigma, np.float64)
+        if X0a.ndim != 2 or X0a.shape[1] != self.dim or Ea.ndim != 2 or Ea.shape[1] != self.dim + 1:
+            raise ValueError("X0 must be [Nverts, dim] and EToV [K, dim+1]")
+        self._check(_lib.alegb_mesh_upload(self._h, X0a.shape[0], X0p, Ea.shape[0], Ep, vp, bp, sp))
+        self.dim, self.N, self.Np, self.Nfp, self.Nfaces, self.Nf, self.K, self.Nverts = self.alegb_get_sizes()
+
+    def alegb_set_params(self, RT, tau, q_inf=None):
+        qa, qp = _host(q_inf, np.float64)
+        self._check(_lib.alegb_set_params(self._h, float(RT), float(tau), qp))
+
+    def alegb_set_motion(self, kind, params=None):
+        pa, pp = _host(params, np.float64)
+        self._check(_lib.alegb_set_motion(self._h, int(kind), pp, 0 if pa is None else pa.size))
+
+    def alegb_set_motion_user(self, d_xv, d_vv):
+        self._check(_lib.alegb_set_motion_user(self._h, _dev(d_xv), _dev(d_vv)))
+
+    # ---- compute (device arrays)
+    def alegb_rhs(self, t, d_q, d_F, stream=None):
+        self._check(_lib.alegb_rhs(self._h, float(t), _dev(d_q), _dev(d_F), _stream(stream)))
+
+    def alegb_rhs_pml(self, t, d_q, d_aux, d_F, d_Faux, stream=None):
+        self._check(_lib.alegb_rhs_pml(self._h, float(t), _dev(d_q), _dev(d_aux), _dev(d_F), _dev(d_Faux), _stream(stream)))
+
+    def alegb_step(self, d_q, t0, dt, nsteps, stream=None):
+        self._check(_lib.alegb_step(self._h, _dev(d_q), float(t0), float(dt), int(nsteps), _stream(stream)))
+
+    def alegb_step_debug(self, d_q, t0, dt, d_stages, stream=None):
+        self._check(_lib.alegb_step_debug(self._h, _dev(d_q), float(t0), float(dt), _dev(d_stages), _stream(stream)))
+
+    def alegb_step_host(self, h_q, t0, dt, nsteps):
+        """h_q: C-contiguous float64 numpy array or CPU torch tensor (pinned or not), updated in place."""
+        ptr = h_q.ctypes.data if isinstance(h_q, np.ndarray) else h_q.data_ptr()
+        self._check(_lib.alegb_step_host(self._h, ptr, float(t0), float(dt), int(nsteps)))
+
+    def alegb_geometry(self, t, d_vgeo=None, d_sgeo=None, d_xv=None, d_vv=None, stream=None):
+        self._check(_lib.alegb_geometry(self._h, float(t), _dev(d_vgeo), _dev(d_sgeo), _dev(d_xv), _dev(d_vv), _stream(stream)))
+
+    # ---- absorbing layer state
+    def alegb_pml_count(self):
+        return int(_lib.alegb_pml_count(self._h))
+
+    def alegb_pml_elements(self):
+        out = np.empty(self.alegb_pml_count(), dtype=np.int32)
+        self._check(_lib.alegb_pml_elements(self._h, out.ctypes.data))
+        return out
+
+    def alegb_pml_reset(self, stream=None):
+        self._check(_lib.alegb_pml_reset(self._h, _stream(stream)))
+
+    def alegb_pml_get(self, d_aux, stream=None):
+        self._check(_lib.alegb_pml_get(self._h, _dev(d_aux), _stream(stream)))
+
+    def alegb_pml_set(self, d_aux, stream=None):
+        self._check(_lib.alegb_pml_set(self._h, _dev(d_aux), _stream(stream)))
+
+    # ---- introspection (host)
+    def alegb_get_sizes(self):
+        ints = [_c.c_int() for _ in range(6)]
+        longs = [_c.c_int64() for _ in range(2)]
+        rc = _lib.alegb_get_sizes(self._h, *[ctypes.byref(v) for v in ints + longs])
+        if rc != OK:
+            raise AlegbError(rc, "alegb_get_sizes")
+        return tuple(int(v.value) for v in ints + longs)
+
+    def alegb_get_operators(self, with_maps=False):
+        Np, ncol = self.Np, self.Nfaces * self.Nfp
+        out = dict(r=np.empty(Np), s=np.empty(Np), t=np.empty(Np) if self.dim == 3 else None,
+                   Dr=np.empty((Np, Np)), Ds=np.empty((Np, Np)), Dt=np.empty((Np, Np)) if self.dim == 3 else None,
+                   LIFT=np.empty((Np, ncol)))
+        maps = dict(vmapM=None, vmapP=None)
+        if with_maps:
+            maps = dict(vmapM=np.empty((self.K, self.Nfaces, self.Nfp), dtype=np.int32),
+                        vmapP=np.empty((self.K, self.Nfaces, self.Nfp), dtype=np.int32))
+        ptr = lambda a: None if a is None else a.ctypes.data
+        self._check(_lib.alegb_get_operators(self._h, ptr(out["r"]), ptr(out["s"]), ptr(out["t"]), ptr(out["Dr"]),
+                                             ptr(out["Ds"]), ptr(out["Dt"]), ptr(out["LIFT"]), ptr(maps["vmapM"]),
+                                             ptr(maps["vmapP"])))
+        out.update(maps)
+        return out
+
+    def alegb_get_reference(self):
+        w = np.empty(self.Np)
+        lam = np.empty((self.Np, self.dim + 1))
+        fmask = np.empty((self.Nfaces, self.Nfp), dtype=np.int32)
+        self._check(_lib.alegb_get_reference(self._h, w.ctypes.data, lam.ctypes.data, fmask.ctypes.data))
+        return dict(w=w, lam=lam, fmask=fmask)
+
+    def alegb_workspace_bytes(self):
+        return int(_lib.alegb_workspace_bytes(self._h))
+
+    def alegb_launch_count(self):
+        return int(_lib.alegb_launch_count(self._h))
+
+    def alegb_last_error(self):
+        return (_lib.alegb_last_error(self._h) or b"").decode()
+
+
+def alegb_sark_coefficients(gamma):
+    a = np.empty(6)
+    b = np.empty(4)
+    rc = _lib.alegb_sark_coefficients(float(gamma), a.ctypes.data, b.ctypes.data)
+    if rc != OK:
+        raise AlegbError(rc, "alegb_sark_coefficients")
+    return a, b
+
+
+def context_from_config(cfg, cuda_device=0):
+    """Create a context and apply mesh / params / motion from a workload dict (workloads/configs.py)."""
+    ctx = Context(cfg["dim"], cfg["N"], cuda_device)
+    ctx.alegb_mesh_upload(cfg["X0"], cfg["EToV"], cfg.get("vertex_equiv"), cfg.get("EToB"), cfg.get("pml_sigma"))
+    ctx.alegb_set_params(cfg["RT"], cfg["tau"], cfg.get("q_inf"))
+    ctx.alegb_set_motion(cfg["motion_kind"], cfg.get("motion_params"))
+    return ctx

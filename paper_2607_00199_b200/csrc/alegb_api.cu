@@ -1,0 +1,573 @@
+// C-ABI entry points (include/alegb.h): context management, mesh upload, the stage loop of the SARK4 step.
+// Host logic only: every arithmetic step of the path runs in the kernels of kernels.cu / stage_mma.cu.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+
+#include "../../include/alegb.h"
+#include "alegb_internal.h"
+
+using namespace alegb;
+
+struct alegb_ctx {
+  int device = 0, num_sms = 0;
+  RefElement ref;
+  int Nf = 0;
+  int64_t K = 0, Nverts = 0, Kpml = 0;
+  bool mesh_ready = false, params_ready = false, has_boundary = false;
+  double RT = 1.0, tau = 1.0, c = 1.0, invtau = 1.0;
+  double q_inf[kMaxFields] = {0};
+  MotionArgs motion{};
+  std::vector<int32_t> vmapM_host, vmapP_host, pml_elems_host;
+  // device: operators
+  double *d_Dt = nullptr, *d_LIFTt = nullptr, *d_lam = nullptr;
+  int32_t* d_fmask = nullptr;
+  // device: mesh
+  double *d_X0 = nullptr, *d_xv = nullptr, *d_vv = nullptr;
+  int32_t *d_EToV = nullptr, *d_vmapP = nullptr;
+  int8_t* d_EToB = nullptr;
+  double *d_vgeo = nullptr, *d_sgeo = nullptr, *d_vvel = nullptr;
+  int32_t *d_pml_index = nullptr, *d_pml_elems = nullptr;
+  double* d_pml_sigma = nullptr;
+  // device: step workspace
+  double *d_Q1 = nullptr, *d_Q2 = nullptr, *d_F0 = nullptr, *d_ACC = nullptr, *d_Qhost = nullptr;
+  double *d_AUX = nullptr, *d_AUXS = nullptr, *d_AUXACC = nullptr;
+  int64_t workspace_bytes = 0;
+  int64_t launches = 0;
+  std::string err;
+};
+
+namespace {
+
+int fail(alegb_ctx* ctx, int code, const std::string& msg) {
+  if (ctx) ctx->err = msg;
+  return code;
+}
+int cuda_fail(alegb_ctx* ctx, cudaError_t e, const char* where) {
+  return fail(ctx, ALEGB_CUDA_ERROR, std::string(where) + ": " + cudaGetErrorString(e));
+}
+#define CU(call)                                             \
+  do {                                                       \
+    cudaError_t e_ = (call);                                 \
+    if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call); \
+  } while (0)
+
+template <class T>
+cudaError_t dev_alloc(alegb_ctx* ctx, T** p, size_t count) {
+  *p = nullptr;
+  if (count == 0) return cudaSuccess;
+  cudaError_t e = cudaMalloc((void**)p, count * sizeof(T));
+  if (e == cudaSuccess) ctx->workspace_bytes += (int64_t)(count * sizeof(T));
+  return e;
+}
+template <class T>
+cudaError_t upload(alegb_ctx* ctx, T** p, const T* host, size_t count) {
+  cudaError_t e = dev_alloc(ctx, p, count);
+  if (e != cudaSuccess || count == 0) return e;
+  return cudaMemcpy(*p, host, count * sizeof(T), cudaMemcpyHostToDevice);
+}
+template <class T>
+void dev_free(T*& p) {
+  if (p) cudaFree(p);
+  p = nullptr;
+}
+
+void free_mesh(alegb_ctx* ctx) {
+  dev_free(ctx->d_X0); dev_free(ctx->d_xv); dev_free(ctx->d_vv); dev_free(ctx->d_EToV); dev_free(ctx->d_vmapP);
+  dev_free(ctx->d_EToB); dev_free(ctx->d_vgeo); dev_free(ctx->d_sgeo); dev_free(ctx->d_vvel);
+  dev_free(ctx->d_pml_index); dev_free(ctx->d_pml_elems); dev_free(ctx->d_pml_sigma);
+  dev_free(ctx->d_Q1); dev_free(ctx->d_Q2); dev_free(ctx->d_F0); dev_free(ctx->d_ACC); dev_free(ctx->d_Qhost);
+  dev_free(ctx->d_AUX); dev_free(ctx->d_AUXS); dev_free(ctx->d_AUXACC);
+  ctx->mesh_ready = false;
+  ctx->K = ctx->Nverts = ctx->Kpml = 0;
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+// a1 + a2 at time t into the context's geometry arrays
+int update_geometry(alegb_ctx* ctx, double t, cudaStream_t s) {
+  const int dim = ctx->ref.dim;
+  if (ctx->motion.kind != ALEGB_MOTION_USER) {
+    CU(launch_vertex_motion(dim, ctx->Nverts, ctx->d_X0, ctx->motion, t, ctx->d_xv, ctx->d_vv, s));
+    ctx->launches++;
+  }
+  CU(launch_geometry(dim, ctx->K, ctx->d_EToV, ctx->d_xv, ctx->d_vv, ctx->d_vgeo, ctx->d_sgeo, ctx->d_vvel, s));
+  ctx->launches++;
+  return ALEGB_OK;
+}
+
+void fill_common(const alegb_ctx* ctx, StageArgs& a) {
+  std::memset(&a, 0, sizeof(a));
+  a.K = ctx->K;
+  a.vgeo = ctx->d_vgeo; a.sgeo = ctx->d_sgeo; a.vvel = ctx->d_vvel;
+  a.vmapP = ctx->d_vmapP; a.EToB = ctx->d_EToB;
+  a.pml_index = ctx->d_pml_index; a.pml_sigma = ctx->d_pml_sigma;
+  a.Dt_ops = ctx->d_Dt; a.LIFTt = ctx->d_LIFTt; a.lam = ctx->d_lam; a.fmask = ctx->d_fmask;
+  a.c = ctx->c; a.invtau = ctx->invtau;
+  for (int k = 0; k < kMaxFields; ++k) a.q_inf[k] = ctx->q_inf[k];
+}
+void fill_common(const alegb_ctx* ctx, PmlArgs& a) {
+  std::memset(&a, 0, sizeof(a));
+  a.Kpml = ctx->Kpml; a.pml_elems = ctx->d_pml_elems; a.pml_sigma = ctx->d_pml_sigma;
+  a.vgeo = ctx->d_vgeo; a.sgeo = ctx->d_sgeo; a.vvel = ctx->d_vvel;
+  a.vmapP = ctx->d_vmapP; a.EToB = ctx->d_EToB;
+  a.Dt_ops = ctx->d_Dt; a.LIFTt = ctx->d_LIFTt; a.lam = ctx->d_lam; a.fmask = ctx->d_fmask;
+  a.c = ctx->c;
+  for (int k = 0; k < kMaxFields; ++k) a.q_inf[k] = ctx->q_inf[k];
+}
+
+int check_ready(alegb_ctx* ctx) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  if (ctx->device < 0) return fail(ctx, ALEGB_CUDA_ERROR, "host-only context (no CUDA device): there is no CPU fallback");
+  if (!ctx->mesh_ready) return fail(ctx, ALEGB_NOT_READY, "alegb_mesh_upload has not been called");
+  if (!ctx->params_ready) return fail(ctx, ALEGB_NOT_READY, "alegb_set_params has not been called");
+  cudaError_t e = cudaSetDevice(ctx->device);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaSetDevice");
+  return ALEGB_OK;
+}
+
+// One SARK4 step.  q_n: state at t0 (read only); outs[i]: where stage state i+1 is written
+// (outs[3] = q_{n+1}, may alias q_n).
+int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t0, double dt, cudaStream_t s) {
+  const int dim = ctx->ref.dim, N = ctx->ref.N, Nf = ctx->Nf;
+  const double gamma = -dt * ctx->invtau;  // L144
+  double as[6], bs[4], a0[6], b0[4];
+  sark_coefficients(gamma, as, bs);
+  sark_coefficients(0.0, a0, b0);
+  bool stiff[kMaxFields];
+  double e_half[kMaxFields], e_full[kMaxFields];
+  for (int k = 0; k < Nf; ++k) {
+    stiff[k] = k > dim;  // second-order moments (L115)
+    const double lam = stiff[k] ? ctx->invtau : 0.0;
+    e_half[k] = std::exp(-(lam * 0.5) * dt);
+    e_full[k] = std::exp(-(lam * 1.0) * dt);
+  }
+  auto A = [&](int k, int idx) { return stiff[k] ? as[idx] : a0[idx]; };  // idx: 0 a10, 1 a20, 2 a21, 3 a30, 5 a32
+  auto B = [&](int k, int j) { return stiff[k] ? bs[j] : b0[j]; };
+  const double cstage[4] = {0.0, 0.5, 0.5, 1.0};
+  const bool pml = ctx->Kpml > 0;
+  for (int i = 0; i < 4; ++i) {
+    const double ti = t0 + cstage[i] * dt;
+    int rc = update_geometry(ctx, ti, s);
+    if (rc != ALEGB_OK) return rc;
+    StageArgs a;
+    fill_common(ctx, a);
+    a.q_in = i == 0 ? q_n : outs[i - 1];
+    a.q_out = outs[i];
+    a.aux = pml ? (i == 0 ? ctx->d_AUX : ctx->d_AUXS) : nullptr;
+    StageCoef& cf = a.coef;
+    if (i == 0) {
+      a.q_n = q_n; a.F_out = ctx->d_F0;
+      for (int k = 0; k < Nf; ++k) { cf.cq_n[k] = e_half[k]; cf.cq_f[k] = dt * A(k, 0); }
+    } else if (i == 1) {
+      a.q_n = q_n; a.F0_in = ctx->d_F0; a.acc_out = ctx->d_ACC;
+      for (int k = 0; k < Nf; ++k) {
+        cf.cq_n[k] = e_half[k]; cf.cq_f0[k] = dt * A(k, 1); cf.cq_f[k] = dt * A(k, 2);
+        cf.ca_n[k] = e_full[k]; cf.ca_f0[k] = dt * B(k, 0); cf.ca_f[k] = dt * B(k, 1);
+      }
+    } else if (i == 2) {
+      a.q_n = q_n; a.F0_in = ctx->d_F0; a.acc_in = ctx->d_ACC; a.acc_out = ctx->d_ACC;
+      cf.ca_acc = 1.0;
+      for (int k = 0; k < Nf; ++k) {
+        cf.cq_n[k] = e_full[k]; cf.cq_f0[k] = dt * A(k, 3); cf.cq_f[k] = dt * A(k, 5);
+        cf.ca_f[k] = dt * B(k, 2);
+      }
+    } else {
+      a.acc_in = ctx->d_ACC;
+      cf.cq_acc = 1.0;
+      for (int k = 0; k < Nf; ++k) cf.cq_f[k] = dt * B(k, 3);
+    }
+    CU(launch_stage(dim, N, a, ctx->num_sms, s));
+    ctx->launches++;
+    if (pml) {
+      // auxiliary fields: Lambda = 0, classic RK4 weights (reading R12)
+      PmlArgs p;
+      fill_common(ctx, p);
+      p.q_in = a.q_in;
+      p.aux_in = i == 0 ? ctx->d_AUX : ctx->d_AUXS;
+      if (i < 3) {
+        p.aux_n = ctx->d_AUX; p.aux_out = ctx->d_AUXS; p.acc_out = ctx->d_AUXACC;
+        p.cx_n = 1.0; p.cx_g = dt * (i == 2 ? 1.0 : 0.5);
+        if (i == 0) { p.cy_n = 1.0; p.cy_g = dt * (1.0 / 6.0); }
+        else { p.acc_in = ctx->d_AUXACC; p.cy_acc = 1.0; p.cy_g = dt * (1.0 / 3.0); }
+      } else {
+        p.acc_in = ctx->d_AUXACC; p.aux_out = ctx->d_AUX; p.cx_acc = 1.0; p.cx_g = dt * (1.0 / 6.0);
+      }
+      CU(launch_pml(dim, N, p, ctx->num_sms, s));
+      ctx->launches++;
+    }
+  }
+  return ALEGB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int alegb_create(alegb_ctx** out, int dim, int N, int cuda_device) {
+  if (!out) return ALEGB_INVALID_ARG;
+  *out = nullptr;
+  if (dim != 2 && dim != 3) return ALEGB_INVALID_ARG;
+  if (N < 1 || N > ALEGB_MAX_N) return ALEGB_UNSUPPORTED;
+  alegb_ctx* ctx = new (std::nothrow) alegb_ctx();
+  if (!ctx) return ALEGB_INVALID_ARG;
+  std::string err;
+  if (!build_reference(dim, N, ctx->ref, err)) { delete ctx; return ALEGB_INVALID_ARG; }
+  ctx->Nf = dim == 2 ? 6 : 10;
+  ctx->device = cuda_device;
+  ctx->motion.kind = ALEGB_MOTION_NONE;
+  if (cuda_device < 0) {  // host-only context: setup and introspection work, every compute call fails
+    *out = ctx;
+    return ALEGB_OK;
+  }
+  cudaError_t e = cudaSetDevice(cuda_device);
+  cudaDeviceProp prop;
+  if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, cuda_device);
+  if (e == cudaSuccess) e = configure_kernels(dim, N);
+  if (e != cudaSuccess) { delete ctx; return ALEGB_CUDA_ERROR; }
+  ctx->num_sms = prop.multiProcessorCount;
+  const RefElement& r = ctx->ref;
+  const int Np = r.Np, ncol = r.Nfaces * r.Nfp;
+  std::vector<double> Dt((size_t)dim * Np * Np), Lt((size_t)ncol * Np);
+  for (int a = 0; a < dim; ++a)
+    for (int i = 0; i < Np; ++i)
+      for (int j = 0; j < Np; ++j) Dt[((size_t)a * Np + j) * Np + i] = r.D[a][i * Np + j];
+  for (int i = 0; i < Np; ++i)
+    for (int m = 0; m < ncol; ++m) Lt[(size_t)m * Np + i] = r.LIFT[i * ncol + m];
+  std::vector<int32_t> fm(r.fmask.begin(), r.fmask.end());
+  if (upload(ctx, &ctx->d_Dt, Dt.data(), Dt.size()) != cudaSuccess ||
+      upload(ctx, &ctx->d_LIFTt, Lt.data(), Lt.size()) != cudaSuccess ||
+      upload(ctx, &ctx->d_lam, r.lam.data(), r.lam.size()) != cudaSuccess ||
+      upload(ctx, &ctx->d_fmask, fm.data(), fm.size()) != cudaSuccess) {
+    alegb_destroy(ctx);
+    return ALEGB_CUDA_ERROR;
+  }
+  *out = ctx;
+  return ALEGB_OK;
+}
+
+int alegb_destroy(alegb_ctx* ctx) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  if (ctx->device >= 0) {
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+  }
+  free_mesh(ctx);
+  dev_free(ctx->d_Dt); dev_free(ctx->d_LIFTt); dev_free(ctx->d_lam); dev_free(ctx->d_fmask);
+  delete ctx;
+  return ALEGB_OK;
+}
+
+int alegb_mesh_upload(alegb_ctx* ctx, int64_t Nverts, const double* X0, int64_t K, const int32_t* EToV,
+                      const int32_t* vertex_equiv, const int8_t* EToB, const double* pml_sigma) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  if (!X0 || !EToV || Nverts <= 0 || K <= 0) return fail(ctx, ALEGB_INVALID_ARG, "X0/EToV missing or empty mesh");
+  if (ctx->device >= 0) CU(cudaSetDevice(ctx->device));
+  const RefElement& r = ctx->ref;
+  const int dim = r.dim, nv = dim + 1, Np = r.Np, Nf = ctx->Nf;
+  for (int64_t i = 0; i < K * nv; ++i)
+    if (EToV[i] < 0 || EToV[i] >= Nverts) return fail(ctx, ALEGB_BAD_MESH, "EToV entry out of range");
+  if (vertex_equiv)
+    for (int64_t i = 0; i < Nverts; ++i)
+      if (vertex_equiv[i] < 0 || vertex_equiv[i] >= Nverts) return fail(ctx, ALEGB_BAD_MESH, "vertex_equiv entry out of range");
+  // positive orientation at t = 0 (L73)
+  for (int64_t e = 0; e < K; ++e) {
+    double G[3][3];
+    for (int a = 0; a < dim; ++a)
+      for (int d = 0; d < dim; ++d) G[d][a] = 0.5 * (X0[(int64_t)EToV[e * nv + a + 1] * dim + d] - X0[(int64_t)EToV[e * nv] * dim + d]);
+    double J = dim == 2 ? G[0][0] * G[1][1] - G[0][1] * G[1][0]
+                        : G[0][0] * (G[1][1] * G[2][2] - G[1][2] * G[2][1]) - G[0][1] * (G[1][0] * G[2][2] - G[1][2] * G[2][0]) +
+                              G[0][2] * (G[1][0] * G[2][1] - G[1][1] * G[2][0]);
+    if (!(J > 0.0)) return fail(ctx, ALEGB_BAD_MESH, "element " + std::to_string(e) + " has a non-positive Jacobian at t = 0");
+  }
+  Connectivity conn;
+  std::string err;
+  int rc = build_connectivity(r, K, EToV, vertex_equiv, EToB, conn, err);
+  if (rc != 0) return fail(ctx, ALEGB_BAD_MESH, err);
+  free_mesh(ctx);
+  ctx->K = K; ctx->Nverts = Nverts;
+  bool any_tag = false;
+  if (EToB) for (int64_t i = 0; i < K * nv; ++i) any_tag |= EToB[i] != 0;
+  ctx->has_boundary = any_tag;
+  // absorbing layer: compact list of flagged elements
+  std::vector<int32_t> pml_index;
+  std::vector<double> sig;
+  ctx->pml_elems_host.clear();
+  if (pml_sigma) {
+    pml_index.assign(K, -1);
+    for (int64_t e = 0; e < K; ++e) {
+      bool in = false;
+      for (int d = 0; d < dim; ++d) {
+        if (pml_sigma[e * dim + d] < 0.0) return fail(ctx, ALEGB_INVALID_ARG, "negative pml_sigma");
+        in |= pml_sigma[e * dim + d] > 0.0;
+      }
+      if (in) {
+        pml_index[e] = (int32_t)ctx->pml_elems_host.size();
+        ctx->pml_elems_host.push_back((int32_t)e);
+        for (int d = 0; d < dim; ++d) sig.push_back(pml_sigma[e * dim + d]);
+      }
+    }
+  }
+  ctx->Kpml = (int64_t)ctx->pml_elems_host.size();
+  ctx->vmapM_host = conn.vmapM; ctx->vmapP_host = conn.vmapP;
+  if (ctx->device < 0) {  // host-only context: connectivity is available for introspection, nothing else
+    ctx->mesh_ready = true;
+    return ALEGB_OK;
+  }
+  const size_t state = (size_t)K * Nf * Np;
+  CU(upload(ctx, &ctx->d_X0, X0, (size_t)Nverts * dim));
+  CU(dev_alloc(ctx, &ctx->d_xv, (size_t)Nverts * dim));
+  CU(dev_alloc(ctx, &ctx->d_vv, (size_t)Nverts * dim));
+  CU(upload(ctx, &ctx->d_EToV, EToV, (size_t)K * nv));
+  CU(upload(ctx, &ctx->d_vmapP, conn.vmapP.data(), conn.vmapP.size()));
+  if (any_tag) CU(upload(ctx, &ctx->d_EToB, EToB, (size_t)K * nv));
+  CU(dev_alloc(ctx, &ctx->d_vgeo, (size_t)K * (dim * dim + 1)));
+  CU(dev_alloc(ctx, &ctx->d_sgeo, (size_t)K * nv * (dim + 2)));
+  CU(dev_alloc(ctx, &ctx->d_vvel, (size_t)K * nv * dim));
+  CU(dev_alloc(ctx, &ctx->d_Q1, state));
+  CU(dev_alloc(ctx, &ctx->d_Q2, state));
+  CU(dev_alloc(ctx, &ctx->d_F0, state));
+  CU(dev_alloc(ctx, &ctx->d_ACC, state));
+  if (ctx->Kpml > 0) {
+    const size_t na = (size_t)ctx->Kpml * dim * Nf * Np;
+    CU(upload(ctx, &ctx->d_pml_index, pml_index.data(), pml_index.size()));
+    CU(upload(ctx, &ctx->d_pml_elems, ctx->pml_elems_host.data(), ctx->pml_elems_host.size()));
+    CU(upload(ctx, &ctx->d_pml_sigma, sig.data(), sig.size()));
+    CU(dev_alloc(ctx, &ctx->d_AUX, na));
+    CU(dev_alloc(ctx, &ctx->d_AUXS, na));
+    CU(dev_alloc(ctx, &ctx->d_AUXACC, na));
+    CU(cudaMemset(ctx->d_AUX, 0, na * sizeof(double)));
+  }
+  CU(cudaMemcpy(ctx->d_xv, ctx->d_X0, (size_t)Nverts * dim * sizeof(double), cudaMemcpyDeviceToDevice));
+  CU(cudaMemset(ctx->d_vv, 0, (size_t)Nverts * dim * sizeof(double)));
+  CU(cudaDeviceSynchronize());
+  ctx->mesh_ready = true;
+  return ALEGB_OK;
+}
+
+int alegb_set_params(alegb_ctx* ctx, double RT, double tau, const double* q_inf) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  if (!(RT > 0.0) || !(tau > 0.0)) return fail(ctx, ALEGB_INVALID_ARG, "RT and tau must be positive");
+  ctx->RT = RT; ctx->tau = tau; ctx->c = std::sqrt(RT);
+  ctx->invtau = std::isinf(tau) ? 0.0 : 1.0 / tau;
+  for (int k = 0; k < kMaxFields; ++k) ctx->q_inf[k] = 0.0;
+  if (q_inf) for (int k = 0; k < ctx->Nf; ++k) ctx->q_inf[k] = q_inf[k];
+  ctx->params_ready = true;
+  return ALEGB_OK;
+}
+
+int alegb_set_motion(alegb_ctx* ctx, int kind, const double* params, int nparams) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  const int dim = ctx->ref.dim;
+  int need = 0;
+  switch (kind) {
+    case ALEGB_MOTION_NONE: need = 0; break;
+    case ALEGB_MOTION_SINES_PRODUCT: need = 2 + 2 * dim; break;
+    case ALEGB_MOTION_SINES_CROSS: need = 4; break;
+    case ALEGB_MOTION_PLUNGE_BLEND: need = 5 + dim; break;
+    case ALEGB_MOTION_CARANGIFORM: need = 10; break;
+    default: return fail(ctx, ALEGB_INVALID_ARG, "unknown motion kind (USER is set by alegb_set_motion_user)");
+  }
+  if (nparams < need || (need > 0 && !params)) return fail(ctx, ALEGB_INVALID_ARG, "too few motion parameters");
+  if (kind == ALEGB_MOTION_PLUNGE_BLEND || kind == ALEGB_MOTION_CARANGIFORM) {
+    int axis = (int)params[kind == ALEGB_MOTION_PLUNGE_BLEND ? 4 : 8];
+    if (axis < 0 || axis >= dim) return fail(ctx, ALEGB_INVALID_ARG, "motion axis out of range");
+  }
+  ctx->motion.kind = kind; ctx->motion.nparams = need;
+  for (int i = 0; i < 16; ++i) ctx->motion.p[i] = i < need ? params[i] : 0.0;
+  return ALEGB_OK;
+}
+
+int alegb_set_motion_user(alegb_ctx* ctx, const double* d_xv, const double* d_vv) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  if (ctx->device < 0) return fail(ctx, ALEGB_CUDA_ERROR, "host-only context (no CUDA device)");
+  if (!ctx->mesh_ready) return fail(ctx, ALEGB_NOT_READY, "alegb_mesh_upload has not been called");
+  if (!d_xv || !d_vv) return fail(ctx, ALEGB_INVALID_ARG, "NULL device array");
+  CU(cudaSetDevice(ctx->device));
+  const size_t bytes = (size_t)ctx->Nverts * ctx->ref.dim * sizeof(double);
+  CU(cudaMemcpyAsync(ctx->d_xv, d_xv, bytes, cudaMemcpyDeviceToDevice, 0));
+  CU(cudaMemcpyAsync(ctx->d_vv, d_vv, bytes, cudaMemcpyDeviceToDevice, 0));
+  CU(cudaStreamSynchronize(0));
+  ctx->motion.kind = ALEGB_MOTION_USER;
+  return ALEGB_OK;
+}
+
+int alegb_rhs_pml(alegb_ctx* ctx, double t, const double* d_q, const double* d_aux, double* d_F, double* d_Faux,
+                  void* stream) {
+  int rc = check_ready(ctx);
+  if (rc != ALEGB_OK) return rc;
+  if (!d_q || !d_F) return fail(ctx, ALEGB_INVALID_ARG, "NULL field pointer");
+  if (!aligned16(d_q) || !aligned16(d_F)) return fail(ctx, ALEGB_INVALID_ARG, "field pointers must be 16-byte aligned");
+  cudaStream_t s = (cudaStream_t)stream;
+  rc = update_geometry(ctx, t, s);
+  if (rc != ALEGB_OK) return rc;
+  StageArgs a;
+  fill_common(ctx, a);
+  a.q_in = d_q; a.F_out = d_F;
+  a.aux = ctx->Kpml > 0 ? (d_aux ? d_aux : ctx->d_AUX) : nullptr;
+  CU(launch_stage(ctx->ref.dim, ctx->ref.N, a, ctx->num_sms, s));
+  ctx->launches++;
+  if (d_Faux && ctx->Kpml > 0) {
+    PmlArgs p;
+    fill_common(ctx, p);
+    p.q_in = d_q; p.aux_in = a.aux; p.G_out = d_Faux;
+    CU(launch_pml(ctx->ref.dim, ctx->ref.N, p, ctx->num_sms, s));
+    ctx->launches++;
+  }
+  return ALEGB_OK;
+}
+
+int alegb_rhs(alegb_ctx* ctx, double t, const double* d_q, double* d_F, void* stream) {
+  return alegb_rhs_pml(ctx, t, d_q, nullptr, d_F, nullptr, stream);
+}
+
+int alegb_step(alegb_ctx* ctx, double* d_q, double t0, double dt, int nsteps, void* stream) {
+  int rc = check_ready(ctx);
+  if (rc != ALEGB_OK) return rc;
+  if (!d_q || nsteps < 0) return fail(ctx, ALEGB_INVALID_ARG, "NULL field pointer or negative step count");
+  if (!aligned16(d_q)) return fail(ctx, ALEGB_INVALID_ARG, "field pointers must be 16-byte aligned");
+  cudaStream_t s = (cudaStream_t)stream;
+  double* outs[4] = {ctx->d_Q1, ctx->d_Q2, ctx->d_Q1, d_q};
+  for (int n = 0; n < nsteps; ++n) {
+    rc = sark_step(ctx, d_q, outs, t0 + n * dt, dt, s);
+    if (rc != ALEGB_OK) return rc;
+  }
+  return ALEGB_OK;
+}
+
+int alegb_step_debug(alegb_ctx* ctx, const double* d_q, double t0, double dt, double* d_stages, void* stream) {
+  int rc = check_ready(ctx);
+  if (rc != ALEGB_OK) return rc;
+  if (!d_q || !d_stages) return fail(ctx, ALEGB_INVALID_ARG, "NULL field pointer");
+  if (!aligned16(d_q) || !aligned16(d_stages)) return fail(ctx, ALEGB_INVALID_ARG, "field pointers must be 16-byte aligned");
+  const size_t state = (size_t)ctx->K * ctx->Nf * ctx->ref.Np;
+  double* outs[4] = {d_stages, d_stages + state, d_stages + 2 * state, d_stages + 3 * state};
+  return sark_step(ctx, d_q, outs, t0, dt, (cudaStream_t)stream);
+}
+
+int alegb_step_host(alegb_ctx* ctx, double* h_q, double t0, double dt, int nsteps) {
+  int rc = check_ready(ctx);
+  if (rc != ALEGB_OK) return rc;
+  if (!h_q) return fail(ctx, ALEGB_INVALID_ARG, "NULL host pointer");
+  const size_t state = (size_t)ctx->K * ctx->Nf * ctx->ref.Np;
+  if (!ctx->d_Qhost) CU(dev_alloc(ctx, &ctx->d_Qhost, state));
+  CU(cudaMemcpyAsync(ctx->d_Qhost, h_q, state * sizeof(double), cudaMemcpyHostToDevice, 0));
+  rc = alegb_step(ctx, ctx->d_Qhost, t0, dt, nsteps, nullptr);
+  if (rc != ALEGB_OK) return rc;
+  CU(cudaMemcpyAsync(h_q, ctx->d_Qhost, state * sizeof(double), cudaMemcpyDeviceToHost, 0));
+  CU(cudaStreamSynchronize(0));
+  return ALEGB_OK;
+}
+
+int alegb_geometry(alegb_ctx* ctx, double t, double* d_vgeo, double* d_sgeo, double* d_xv, double* d_vv, void* stream) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  if (ctx->device < 0) return fail(ctx, ALEGB_CUDA_ERROR, "host-only context (no CUDA device)");
+  if (!ctx->mesh_ready) return fail(ctx, ALEGB_NOT_READY, "alegb_mesh_upload has not been called");
+  CU(cudaSetDevice(ctx->device));
+  cudaStream_t s = (cudaStream_t)stream;
+  int rc = update_geometry(ctx, t, s);
+  if (rc != ALEGB_OK) return rc;
+  const int dim = ctx->ref.dim;
+  const size_t K = (size_t)ctx->K, nvb = (size_t)ctx->Nverts * dim * sizeof(double);
+  if (d_vgeo) CU(cudaMemcpyAsync(d_vgeo, ctx->d_vgeo, K * (dim * dim + 1) * sizeof(double), cudaMemcpyDeviceToDevice, s));
+  if (d_sgeo) CU(cudaMemcpyAsync(d_sgeo, ctx->d_sgeo, K * (dim + 1) * (dim + 2) * sizeof(double), cudaMemcpyDeviceToDevice, s));
+  if (d_xv) CU(cudaMemcpyAsync(d_xv, ctx->d_xv, nvb, cudaMemcpyDeviceToDevice, s));
+  if (d_vv) CU(cudaMemcpyAsync(d_vv, ctx->d_vv, nvb, cudaMemcpyDeviceToDevice, s));
+  return ALEGB_OK;
+}
+
+int64_t alegb_pml_count(const alegb_ctx* ctx) { return ctx ? ctx->Kpml : 0; }
+
+int alegb_pml_elements(const alegb_ctx* ctx, int32_t* elems) {
+  if (!ctx || !elems) return ALEGB_INVALID_ARG;
+  for (size_t i = 0; i < ctx->pml_elems_host.size(); ++i) elems[i] = ctx->pml_elems_host[i];
+  return ALEGB_OK;
+}
+
+int alegb_pml_reset(alegb_ctx* ctx, void* stream) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  if (ctx->Kpml == 0) return ALEGB_OK;
+  if (ctx->device < 0) return fail(ctx, ALEGB_CUDA_ERROR, "host-only context (no CUDA device)");
+  CU(cudaSetDevice(ctx->device));
+  const size_t na = (size_t)ctx->Kpml * ctx->ref.dim * ctx->Nf * ctx->ref.Np;
+  CU(cudaMemsetAsync(ctx->d_AUX, 0, na * sizeof(double), (cudaStream_t)stream));
+  return ALEGB_OK;
+}
+
+int alegb_pml_get(alegb_ctx* ctx, double* d_aux, void* stream) {
+  if (!ctx || !d_aux) return ALEGB_INVALID_ARG;
+  if (ctx->Kpml == 0) return ALEGB_OK;
+  if (ctx->device < 0) return fail(ctx, ALEGB_CUDA_ERROR, "host-only context (no CUDA device)");
+  CU(cudaSetDevice(ctx->device));
+  const size_t na = (size_t)ctx->Kpml * ctx->ref.dim * ctx->Nf * ctx->ref.Np;
+  CU(cudaMemcpyAsync(d_aux, ctx->d_AUX, na * sizeof(double), cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  return ALEGB_OK;
+}
+
+int alegb_pml_set(alegb_ctx* ctx, const double* d_aux, void* stream) {
+  if (!ctx || !d_aux) return ALEGB_INVALID_ARG;
+  if (ctx->Kpml == 0) return ALEGB_OK;
+  if (ctx->device < 0) return fail(ctx, ALEGB_CUDA_ERROR, "host-only context (no CUDA device)");
+  CU(cudaSetDevice(ctx->device));
+  const size_t na = (size_t)ctx->Kpml * ctx->ref.dim * ctx->Nf * ctx->ref.Np;
+  CU(cudaMemcpyAsync(ctx->d_AUX, d_aux, na * sizeof(double), cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  return ALEGB_OK;
+}
+
+int alegb_get_sizes(const alegb_ctx* ctx, int* dim, int* N, int* Np, int* Nfp, int* Nfaces, int* Nfields, int64_t* K,
+                    int64_t* Nverts) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  if (dim) *dim = ctx->ref.dim;
+  if (N) *N = ctx->ref.N;
+  if (Np) *Np = ctx->ref.Np;
+  if (Nfp) *Nfp = ctx->ref.Nfp;
+  if (Nfaces) *Nfaces = ctx->ref.Nfaces;
+  if (Nfields) *Nfields = ctx->Nf;
+  if (K) *K = ctx->K;
+  if (Nverts) *Nverts = ctx->Nverts;
+  return ALEGB_OK;
+}
+
+int alegb_get_operators(alegb_ctx* ctx, double* r, double* s, double* t3, double* Dr, double* Ds, double* Dt,
+                        double* LIFT, int32_t* vmapM, int32_t* vmapP) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  const RefElement& R = ctx->ref;
+  const int Np = R.Np;
+  auto cp = [](double* dst, const double* src, size_t n) { if (dst) std::memcpy(dst, src, n * sizeof(double)); };
+  cp(r, R.rst.data(), Np);
+  cp(s, R.rst.data() + Np, Np);
+  if (R.dim == 3) cp(t3, R.rst.data() + 2 * Np, Np);
+  cp(Dr, R.D[0].data(), (size_t)Np * Np);
+  cp(Ds, R.D[1].data(), (size_t)Np * Np);
+  if (R.dim == 3) cp(Dt, R.D[2].data(), (size_t)Np * Np);
+  cp(LIFT, R.LIFT.data(), R.LIFT.size());
+  if (vmapM || vmapP) {
+    if (!ctx->mesh_ready) return fail(ctx, ALEGB_NOT_READY, "alegb_mesh_upload has not been called");
+    if (vmapM) std::memcpy(vmapM, ctx->vmapM_host.data(), ctx->vmapM_host.size() * sizeof(int32_t));
+    if (vmapP) std::memcpy(vmapP, ctx->vmapP_host.data(), ctx->vmapP_host.size() * sizeof(int32_t));
+  }
+  return ALEGB_OK;
+}
+
+int alegb_get_reference(const alegb_ctx* ctx, double* w, double* lam, int32_t* fmask) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  const RefElement& R = ctx->ref;
+  if (w) std::memcpy(w, R.w.data(), R.w.size() * sizeof(double));
+  if (lam) std::memcpy(lam, R.lam.data(), R.lam.size() * sizeof(double));
+  if (fmask) for (size_t i = 0; i < R.fmask.size(); ++i) fmask[i] = R.fmask[i];
+  return ALEGB_OK;
+}
+
+int alegb_sark_coefficients(double gamma, double* a, double* b) {
+  if (!a || !b) return ALEGB_INVALID_ARG;
+  sark_coefficients(gamma, a, b);
+  return ALEGB_OK;
+}
+
+int64_t alegb_workspace_bytes(const alegb_ctx* ctx) { return ctx ? ctx->workspace_bytes : 0; }
+const char* alegb_last_error(const alegb_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+int64_t alegb_launch_count(const alegb_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+}  // extern "C"

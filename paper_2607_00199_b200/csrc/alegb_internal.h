@@ -1,0 +1,89 @@
+// Internal declarations shared by the library's translation units (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "host_ref.h"
+
+namespace alegb {
+
+constexpr int kMaxFields = 10;
+
+// Per-field coefficients of one fused stage (PAPER.md:L132-134 written as two linear combinations):
+//   q_out   = cq_n  q_n + cq_f0 F0 + cq_acc acc_in + cq_f F
+//   acc_out = ca_n  q_n + ca_f0 F0 + ca_acc acc_in + ca_f F
+// F is the operator of eq. 9 evaluated on q_in at the stage time.  A NULL output pointer skips that output; inputs
+// whose coefficients are all zero are not read.
+struct StageCoef {
+  double cq_n[kMaxFields], cq_f0[kMaxFields], cq_f[kMaxFields];
+  double ca_n[kMaxFields], ca_f0[kMaxFields], ca_f[kMaxFields];
+  double cq_acc, ca_acc;
+};
+
+struct StageArgs {
+  // mesh / geometry at the stage time
+  int64_t K;
+  const double* vgeo;    // [K][dim*dim+1]
+  const double* sgeo;    // [K][Nfaces][dim+2]
+  const double* vvel;    // [K][dim+1][dim] vertex velocities of each element
+  const int32_t* vmapP;  // [K][Nfaces*Nfp]
+  const int8_t* EToB;    // [K][Nfaces] or NULL
+  const int32_t* pml_index;  // [K] index into the auxiliary arrays, -1 outside the layer; or NULL
+  const double* pml_sigma;   // [Kpml][dim]
+  const double* aux;         // [Kpml][dim][Nf][Np] auxiliary state entering F, or NULL
+  // operators (device, transposed for coalesced staging)
+  const double* Dt_ops;  // [dim][Np(j)][Np(i)] : D_a[i][j]
+  const double* LIFTt;   // [Nfaces*Nfp(m)][Np(i)] : LIFT[i][m]
+  const double* lam;     // [Np][dim+1]
+  const int32_t* fmask;  // [Nfaces*Nfp]
+  // physics
+  double c, invtau;
+  double q_inf[kMaxFields];
+  // fields
+  const double* q_in;
+  const double* q_n;
+  const double* F0_in;
+  const double* acc_in;
+  double* F_out;    // plain F (stage 0 writes F0 here; rhs mode writes the result here)
+  double* q_out;
+  double* acc_out;
+  StageCoef coef;
+};
+
+struct PmlArgs {
+  int64_t Kpml;
+  const int32_t* pml_elems;  // [Kpml]
+  const double* pml_sigma;   // [Kpml][dim]
+  const double* vgeo; const double* sgeo; const double* vvel;
+  const int32_t* vmapP; const int8_t* EToB;
+  const double* Dt_ops; const double* LIFTt; const double* lam; const int32_t* fmask;
+  double c;
+  double q_inf[kMaxFields];
+  const double* q_in;
+  // auxiliary fields [Kpml][dim][Nf][Np]:  G = rhs of the auxiliary equation (reading R12)
+  //   aux_out = cx_n aux_n + cx_acc acc_in + cx_g G ;  acc_out = cy_n aux_n + cy_acc acc_in + cy_g G
+  const double* aux_in;   // state G is evaluated on
+  const double* aux_n; const double* acc_in;
+  double* G_out; double* aux_out; double* acc_out;
+  double cx_n, cx_acc, cx_g, cy_n, cy_acc, cy_g;
+};
+
+struct MotionArgs {
+  int kind; int nparams;
+  double p[16];
+};
+
+// kernel launchers (kernels.cu); return cudaGetLastError()
+cudaError_t launch_vertex_motion(int dim, int64_t Nverts, const double* X0, const MotionArgs& m, double t, double* xv,
+                                 double* vv, cudaStream_t s);
+cudaError_t launch_geometry(int dim, int64_t K, const int32_t* EToV, const double* xv, const double* vv, double* vgeo,
+                            double* sgeo, double* vvel, cudaStream_t s);
+// returns cudaErrorInvalidValue if (dim, N) has no compiled kernel
+cudaError_t launch_stage(int dim, int N, const StageArgs& a, int num_sms, cudaStream_t s);
+cudaError_t launch_pml(int dim, int N, const PmlArgs& a, int num_sms, cudaStream_t s);
+cudaError_t configure_kernels(int dim, int N);
+
+}  // namespace alegb

@@ -1,0 +1,488 @@
+// CUDA kernels of the ALE Galerkin-Boltzmann stage (sm_100a), generic element-blocked path for every (dim, N).
+//
+//   a1  vertex_motion_kernel   positions / velocities of the vertices from the prescribed law
+//   a2  geometry_kernel        geometric factors of the moved affine simplices (L88-92, L193)
+//   a3-a6 stage_kernel         volume + collocated relaxation + surface + SARK stage update, fused (L107, L132-134)
+//   a8  pml_kernel             auxiliary fields of the absorbing layer (reading R12)
+//
+// The tensor-core (DMMA) specialisations of the stage kernel live in stage_mma.cu.
+#include <cstdio>
+
+#include "alegb_internal.h"
+#include "device_common.cuh"
+
+namespace alegb {
+
+// ------------------------------------------------------------------------------------------------------------------
+// a1: vertex motion.  One thread per vertex.
+template <int DIM>
+__global__ void vertex_motion_kernel(int64_t Nverts, const double* __restrict__ X0, MotionArgs m, double t,
+                                     double* __restrict__ xv, double* __restrict__ vv) {
+  int64_t v = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (v >= Nverts) return;
+  double X[DIM], disp[DIM], vel[DIM];
+#pragma unroll
+  for (int d = 0; d < DIM; ++d) { X[d] = X0[v * DIM + d]; disp[d] = 0.0; vel[d] = 0.0; }
+  const double* p = m.p;
+  if (m.kind == 1) {  // SINES_PRODUCT: eq. 15
+    double A = p[0], om = 2.0 * M_PI / p[1], shape = 1.0;
+#pragma unroll
+    for (int d = 0; d < DIM; ++d) shape *= sin(p[2 + d] * X[d] + p[2 + DIM + d]);
+    double s = A * sin(om * t) * shape, ds = A * om * cos(om * t) * shape;
+#pragma unroll
+    for (int d = 0; d < DIM; ++d) { disp[d] = s; vel[d] = ds; }
+  } else if (m.kind == 2) {  // SINES_CROSS: eq. 19
+    double A = p[0], om = 2.0 * M_PI / p[1], k = p[2], ph = p[3];
+    double sn[DIM];
+#pragma unroll
+    for (int d = 0; d < DIM; ++d) sn[d] = sin(k * X[d] + ph);
+#pragma unroll
+    for (int d = 0; d < DIM; ++d) {
+      double shape = 1.0;
+#pragma unroll
+      for (int o = 0; o < DIM; ++o) if (o != d) shape *= sn[o];
+      disp[d] = A * sin(om * t) * shape;
+      vel[d] = A * om * cos(om * t) * shape;
+    }
+  } else if (m.kind == 3) {  // PLUNGE_BLEND: eqs. 20-21 times a radial quintic blend
+    double h0 = p[0], om = p[1], r1 = p[2], r2 = p[3];
+    int axis = (int)p[4];
+    double rho2 = 0.0;
+#pragma unroll
+    for (int d = 0; d < DIM; ++d) rho2 += (X[d] - p[5 + d]) * (X[d] - p[5 + d]);
+    double u = (sqrt(rho2) - r1) / (r2 - r1);
+    u = fmin(fmax(u, 0.0), 1.0);
+    double b = 1.0 - (6.0 * u * u * u * u * u - 15.0 * u * u * u * u + 10.0 * u * u * u);
+#pragma unroll
+    for (int d = 0; d < DIM; ++d)
+      if (d == axis) { disp[d] = h0 * sin(om * t) * b; vel[d] = h0 * om * cos(om * t) * b; }
+  } else if (m.kind == 4) {  // CARANGIFORM: L339-365
+    double a0 = p[0], a1 = p[1], a2 = p[2], k = p[3], om = p[4], Rr = p[5], beta = p[6], Tr = p[7];
+    int axis = (int)p[8];
+    double Bcut = p[9];
+    double xt = fmin(1.0, fmax(0.0, X[0]));
+    double r2 = (X[0] - xt) * (X[0] - xt);
+#pragma unroll
+    for (int d = 1; d < DIM; ++d) r2 += X[d] * X[d];
+    double deff = fmax(sqrt(r2) - Rr, 0.0);
+    double B = exp(-beta * deff * deff);
+    if (B < Bcut) B = 0.0;
+    double Amp = a0 + a1 * xt + a2 * xt * xt;
+    double phi = k * X[0] - om * t;
+    double S = 1.0, Sd = 0.0;
+    if (t < Tr) { S = 0.5 * (1.0 - cos(M_PI * t / Tr)); Sd = M_PI / (2.0 * Tr) * sin(M_PI * t / Tr); }
+#pragma unroll
+    for (int d = 0; d < DIM; ++d)
+      if (d == axis) {
+        disp[d] = Amp * sin(phi) * B * S;
+        vel[d] = -Amp * om * cos(phi) * B * S + Amp * sin(phi) * B * Sd;
+      }
+  }
+#pragma unroll
+  for (int d = 0; d < DIM; ++d) { xv[v * DIM + d] = X[d] + disp[d]; vv[v * DIM + d] = vel[d]; }
+}
+
+cudaError_t launch_vertex_motion(int dim, int64_t Nverts, const double* X0, const MotionArgs& m, double t, double* xv,
+                                 double* vv, cudaStream_t s) {
+  if (Nverts == 0) return cudaSuccess;
+  int nb = (int)((Nverts + 255) / 256);
+  if (dim == 2) vertex_motion_kernel<2><<<nb, 256, 0, s>>>(Nverts, X0, m, t, xv, vv);
+  else vertex_motion_kernel<3><<<nb, 256, 0, s>>>(Nverts, X0, m, t, xv, vv);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// a2: geometric factors.  One thread per element, registers only (as PAPER.md:L193).
+template <int DIM>
+__global__ void geometry_kernel(int64_t K, const int32_t* __restrict__ EToV, const double* __restrict__ xv,
+                                const double* __restrict__ vv, double* __restrict__ vgeo, double* __restrict__ sgeo,
+                                double* __restrict__ vvel) {
+  int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (e >= K) return;
+  double X[DIM + 1][DIM];
+#pragma unroll
+  for (int v = 0; v <= DIM; ++v) {
+    int64_t id = EToV[e * (DIM + 1) + v];
+#pragma unroll
+    for (int d = 0; d < DIM; ++d) {
+      X[v][d] = xv[id * DIM + d];
+      if (vvel) vvel[(e * (DIM + 1) + v) * DIM + d] = vv[id * DIM + d];
+    }
+  }
+  double vg[DIM * DIM + 1], sg[(DIM + 1) * (DIM + 2)];
+  element_geometry<DIM>(X, vg, sg);
+  if (vgeo)
+#pragma unroll
+    for (int i = 0; i < DIM * DIM + 1; ++i) vgeo[e * (DIM * DIM + 1) + i] = vg[i];
+  if (sgeo)
+#pragma unroll
+    for (int i = 0; i < (DIM + 1) * (DIM + 2); ++i) sgeo[e * (DIM + 1) * (DIM + 2) + i] = sg[i];
+}
+
+cudaError_t launch_geometry(int dim, int64_t K, const int32_t* EToV, const double* xv, const double* vv, double* vgeo,
+                            double* sgeo, double* vvel, cudaStream_t s) {
+  if (K == 0) return cudaSuccess;
+  int nb = (int)((K + 127) / 128);
+  if (dim == 2) geometry_kernel<2><<<nb, 128, 0, s>>>(K, EToV, xv, vv, vgeo, sgeo, vvel);
+  else geometry_kernel<3><<<nb, 128, 0, s>>>(K, EToV, xv, vv, vgeo, sgeo, vvel);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// a3-a6: fused stage, generic path.  A persistent CTA stages the operator matrices in shared memory once and loops
+// over batches of EB consecutive elements; thread = (element in batch, node).
+template <int DIM, int N>
+struct StageCfg {
+  static constexpr int Np = DIM == 2 ? (N + 1) * (N + 2) / 2 : (N + 1) * (N + 2) * (N + 3) / 6;
+  static constexpr int Nfp = DIM == 2 ? N + 1 : (N + 1) * (N + 2) / 2;
+  static constexpr int Nfaces = DIM + 1;
+  static constexpr int NFN = Nfaces * Nfp;
+  static constexpr int Nf = DIM == 2 ? 6 : 10;
+  static constexpr int EB = (256 / Np) > 0 ? (256 / Np) : 1;
+  static constexpr int Threads = EB * Np;
+  static constexpr size_t smem_doubles = (size_t)DIM * Np * Np + (size_t)NFN * Np + (size_t)EB * Nf * Np +
+                                         (size_t)EB * Nf * NFN + (size_t)Np * (DIM + 1);
+  static constexpr size_t smem_bytes = smem_doubles * 8 + (size_t)NFN * 4;
+};
+
+// trace state q+ on a face node, including the boundary states of reading R11
+template <int DIM>
+__device__ __forceinline__ void exterior_state(int tag, const double* qM, const double* vG, double c,
+                                               const double* q_inf, double* qP) {
+  constexpr int Nf = DIM == 2 ? 6 : 10;
+  if (tag == 1) {  // wall moving with the mesh
+#pragma unroll
+    for (int k = 0; k < Nf; ++k) qP[k] = qM[k];
+#pragma unroll
+    for (int d = 0; d < DIM; ++d) qP[1 + d] = 2.0 * qM[0] * vG[d] / c - qM[1 + d];
+  } else {  // far field
+#pragma unroll
+    for (int k = 0; k < Nf; ++k) qP[k] = q_inf[k];
+  }
+}
+
+template <int DIM, int N>
+__global__ void __launch_bounds__(StageCfg<DIM, N>::Threads) stage_kernel(StageArgs a) {
+  using C = StageCfg<DIM, N>;
+  constexpr int Np = C::Np, Nfp = C::Nfp, Nfaces = C::Nfaces, NFN = C::NFN, Nf = C::Nf, EB = C::EB;
+  extern __shared__ double smem[];
+  double* sD = smem;                     // [DIM][Np j][Np i]
+  double* sL = sD + DIM * Np * Np;       // [NFN m][Np i]
+  double* sq = sL + NFN * Np;            // [EB][Nf][Np]
+  double* sflux = sq + EB * Nf * Np;     // [EB][Nf][NFN]
+  double* slam = sflux + EB * Nf * NFN;  // [Np][DIM+1]
+  int* sfmask = reinterpret_cast<int*>(slam + Np * (DIM + 1));
+  const int tid = threadIdx.x;
+  for (int x = tid; x < DIM * Np * Np; x += C::Threads) sD[x] = a.Dt_ops[x];
+  for (int x = tid; x < NFN * Np; x += C::Threads) sL[x] = a.LIFTt[x];
+  for (int x = tid; x < Np * (DIM + 1); x += C::Threads) slam[x] = a.lam[x];
+  for (int x = tid; x < NFN; x += C::Threads) sfmask[x] = a.fmask[x];
+  const int el = tid / Np, i = tid - el * Np;
+  const double c = a.c;
+  const int64_t nbatch = (a.K + EB - 1) / EB;
+  for (int64_t batch = blockIdx.x; batch < nbatch; batch += gridDim.x) {
+    const int64_t e0 = batch * EB;
+    const int64_t e = e0 + el;
+    const bool active = e < a.K;
+    __syncthreads();
+    {
+      const int64_t nel = (a.K - e0) < EB ? (a.K - e0) : EB;
+      const int nload = (int)nel * Nf * Np;
+      const double* src = a.q_in + e0 * Nf * Np;
+      for (int x = tid; x < nload; x += C::Threads) sq[x] = src[x];
+    }
+    __syncthreads();
+    double rhs[Nf];
+    if (active) {
+      // ---- a3: reference derivatives, dense Np x Np mat-vecs (L103, L195)
+      double dr[DIM][Nf];
+#pragma unroll
+      for (int d = 0; d < DIM; ++d)
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) dr[d][k] = 0.0;
+      for (int j = 0; j < Np; ++j) {
+        double dm[DIM];
+#pragma unroll
+        for (int d = 0; d < DIM; ++d) dm[d] = sD[(d * Np + j) * Np + i];
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) {
+          double qv = sq[(el * Nf + k) * Np + j];
+#pragma unroll
+          for (int d = 0; d < DIM; ++d) dr[d][k] = fma(dm[d], qv, dr[d][k]);
+        }
+      }
+      const double* vg = a.vgeo + e * (DIM * DIM + 1);
+      double G[DIM][DIM];
+#pragma unroll
+      for (int r = 0; r < DIM; ++r)
+#pragma unroll
+        for (int d = 0; d < DIM; ++d) G[r][d] = vg[r * DIM + d];
+      double vG[DIM];
+      node_velocity<DIM>(slam + i * (DIM + 1), a.vvel + e * (DIM + 1) * DIM, vG);
+      double gr[DIM][Nf];
+#pragma unroll
+      for (int d = 0; d < DIM; ++d)
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) {
+          double s = 0.0;
+#pragma unroll
+          for (int r = 0; r < DIM; ++r) s = fma(G[r][d], dr[r][k], s);
+          gr[d][k] = s;
+        }
+      double st[Nf];
+      hermite_apply<DIM>([&](int d, int j) { return gr[d][j]; }, st);
+      double qn[Nf];
+#pragma unroll
+      for (int k = 0; k < Nf; ++k) qn[k] = sq[(el * Nf + k) * Np + i];
+      double nt[Nf];
+      relaxation<DIM>(qn, a.invtau, nt);  // a4 (L115; reading R8)
+#pragma unroll
+      for (int k = 0; k < Nf; ++k) {
+        double v = -c * st[k];
+#pragma unroll
+        for (int d = 0; d < DIM; ++d) v = fma(vG[d], gr[d][k], v);
+        rhs[k] = v + nt[k];
+      }
+      if (a.pml_index != nullptr && a.aux != nullptr) {
+        int p = a.pml_index[e];
+        if (p >= 0) {
+#pragma unroll
+          for (int d = 0; d < DIM; ++d) {
+            double sig = a.pml_sigma[(int64_t)p * DIM + d];
+#pragma unroll
+            for (int k = 0; k < Nf; ++k) rhs[k] -= sig * a.aux[(((int64_t)p * DIM + d) * Nf + k) * Np + i];
+          }
+        }
+      }
+    }
+    // ---- a5: surface flux at the face nodes of the batch (eq. 7; reading R7)
+    for (int x = tid; x < EB * NFN; x += C::Threads) {
+      const int fe = x / NFN, m = x - fe * NFN;
+      const int64_t ee = e0 + fe;
+      if (ee >= a.K) break;
+      const int f = m / Nfp, n = sfmask[m];
+      double qM[Nf], qP[Nf];
+#pragma unroll
+      for (int k = 0; k < Nf; ++k) qM[k] = sq[(fe * Nf + k) * Np + n];
+      const double* sg = a.sgeo + (ee * Nfaces + f) * (DIM + 2);
+      double nh[DIM], vG[DIM];
+#pragma unroll
+      for (int d = 0; d < DIM; ++d) nh[d] = sg[d];
+      const double Fscale = sg[DIM + 1];
+      node_velocity<DIM>(slam + n * (DIM + 1), a.vvel + ee * (DIM + 1) * DIM, vG);
+      const int tag = a.EToB ? a.EToB[ee * Nfaces + f] : 0;
+      if (tag == 0) {
+        const int idP = a.vmapP[ee * NFN + m];
+        const int eP = idP / Np, nP = idP - eP * Np;
+        const double* qp = a.q_in + (int64_t)eP * Nf * Np + nP;
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) qP[k] = qp[k * Np];
+      } else {
+        exterior_state<DIM>(tag, qM, vG, c, a.q_inf, qP);
+      }
+      double vn = 0.0;
+#pragma unroll
+      for (int d = 0; d < DIM; ++d) vn = fma(vG[d], nh[d], vn);
+      double fl[Nf];
+      upwind_flux<DIM>(qM, qP, nh, c, vn, Fscale, fl);
+#pragma unroll
+      for (int k = 0; k < Nf; ++k) sflux[(fe * Nf + k) * NFN + m] = fl[k];
+    }
+    __syncthreads();
+    if (active) {
+      // ---- LIFT (L103, L196)
+      for (int m = 0; m < NFN; ++m) {
+        double l = sL[m * Np + i];
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) rhs[k] = fma(l, sflux[(el * Nf + k) * NFN + m], rhs[k]);
+      }
+      // ---- a6: SARK stage update (L132-134)
+#pragma unroll
+      for (int k = 0; k < Nf; ++k) {
+        const int64_t idx = (e * Nf + k) * Np + i;
+        stage_update(a, k, idx, rhs[k]);
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// a8: auxiliary fields of the absorbing layer (reading R12), elements of the layer only.
+template <int DIM, int N>
+__global__ void __launch_bounds__(StageCfg<DIM, N>::Threads) pml_kernel(PmlArgs a) {
+  using C = StageCfg<DIM, N>;
+  constexpr int Np = C::Np, Nfp = C::Nfp, Nfaces = C::Nfaces, NFN = C::NFN, Nf = C::Nf, EB = C::EB;
+  extern __shared__ double smem[];
+  double* sD = smem;
+  double* sL = sD + DIM * Np * Np;
+  double* sq = sL + NFN * Np;
+  double* sflux = sq + EB * Nf * Np;
+  double* slam = sflux + EB * Nf * NFN;
+  int* sfmask = reinterpret_cast<int*>(slam + Np * (DIM + 1));
+  const int tid = threadIdx.x;
+  for (int x = tid; x < DIM * Np * Np; x += C::Threads) sD[x] = a.Dt_ops[x];
+  for (int x = tid; x < NFN * Np; x += C::Threads) sL[x] = a.LIFTt[x];
+  for (int x = tid; x < Np * (DIM + 1); x += C::Threads) slam[x] = a.lam[x];
+  for (int x = tid; x < NFN; x += C::Threads) sfmask[x] = a.fmask[x];
+  const int el = tid / Np, i = tid - el * Np;
+  const double c = a.c;
+  const int64_t nbatch = (a.Kpml + EB - 1) / EB;
+  for (int64_t batch = blockIdx.x; batch < nbatch; batch += gridDim.x) {
+    const int64_t p0 = batch * EB;
+    const int64_t p = p0 + el;
+    const bool active = p < a.Kpml;
+    const int64_t e = active ? a.pml_elems[p] : 0;
+    __syncthreads();
+    if (active)
+      for (int k = 0; k < Nf; ++k) sq[(el * Nf + k) * Np + i] = a.q_in[(e * Nf + k) * Np + i];
+    __syncthreads();
+    double gr[DIM][Nf];
+    if (active) {
+      double dr[DIM][Nf];
+#pragma unroll
+      for (int d = 0; d < DIM; ++d)
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) dr[d][k] = 0.0;
+      for (int j = 0; j < Np; ++j) {
+        double dm[DIM];
+#pragma unroll
+        for (int d = 0; d < DIM; ++d) dm[d] = sD[(d * Np + j) * Np + i];
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) {
+          double qv = sq[(el * Nf + k) * Np + j];
+#pragma unroll
+          for (int d = 0; d < DIM; ++d) dr[d][k] = fma(dm[d], qv, dr[d][k]);
+        }
+      }
+      const double* vg = a.vgeo + e * (DIM * DIM + 1);
+#pragma unroll
+      for (int d = 0; d < DIM; ++d)
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) {
+          double s = 0.0;
+#pragma unroll
+          for (int r = 0; r < DIM; ++r) s = fma(vg[r * DIM + d], dr[r][k], s);
+          gr[d][k] = s;
+        }
+    }
+#pragma unroll
+    for (int dd = 0; dd < DIM; ++dd) {
+      __syncthreads();
+      for (int x = tid; x < EB * NFN; x += C::Threads) {
+        const int fe = x / NFN, m = x - fe * NFN;
+        if (p0 + fe >= a.Kpml) break;
+        const int64_t ee = a.pml_elems[p0 + fe];
+        const int f = m / Nfp, n = sfmask[m];
+        double qM[Nf], qP[Nf];
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) qM[k] = sq[(fe * Nf + k) * Np + n];
+        const double* sg = a.sgeo + (ee * Nfaces + f) * (DIM + 2);
+        double nh[DIM];
+#pragma unroll
+        for (int d = 0; d < DIM; ++d) nh[d] = sg[d];
+        const double Fscale = sg[DIM + 1];
+        const int tag = a.EToB ? a.EToB[ee * Nfaces + f] : 0;
+        if (tag == 0) {
+          const int idP = a.vmapP[ee * NFN + m];
+          const int eP = idP / Np, nP = idP - eP * Np;
+          const double* qp = a.q_in + (int64_t)eP * Nf * Np + nP;
+#pragma unroll
+          for (int k = 0; k < Nf; ++k) qP[k] = qp[k * Np];
+        } else {
+          double vG[DIM];
+          node_velocity<DIM>(slam + n * (DIM + 1), a.vvel + ee * (DIM + 1) * DIM, vG);
+          exterior_state<DIM>(tag, qM, vG, c, a.q_inf, qP);
+        }
+        double fl[Nf];
+        directional_flux<DIM>(dd, qM, qP, nh, c, Fscale, fl);
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) sflux[(fe * Nf + k) * NFN + m] = fl[k];
+      }
+      __syncthreads();
+      if (active) {
+        double G[Nf];
+        hermite_apply<DIM>([&](int d, int j) { return d == dd ? gr[dd][j] : 0.0; }, G);
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) G[k] = -c * G[k];
+        for (int m = 0; m < NFN; ++m) {
+          double l = sL[m * Np + i];
+#pragma unroll
+          for (int k = 0; k < Nf; ++k) G[k] = fma(l, sflux[(el * Nf + k) * NFN + m], G[k]);
+        }
+        const double sig = a.pml_sigma[p * DIM + dd];
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) {
+          const int64_t idx = ((p * DIM + dd) * Nf + k) * Np + i;
+          const double g = G[k] - sig * a.aux_in[idx];
+          if (a.G_out) a.G_out[idx] = g;
+          const double xn = a.aux_n ? a.aux_n[idx] : 0.0;
+          const double ac = a.acc_in ? a.acc_in[idx] : 0.0;
+          if (a.aux_out) a.aux_out[idx] = fma(a.cx_g, g, fma(a.cx_acc, ac, a.cx_n * xn));
+          if (a.acc_out) a.acc_out[idx] = fma(a.cy_g, g, fma(a.cy_acc, ac, a.cy_n * xn));
+        }
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+template <int DIM, int N>
+static cudaError_t configure_one() {
+  using C = StageCfg<DIM, N>;
+  cudaError_t err = cudaFuncSetAttribute(stage_kernel<DIM, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
+  if (err != cudaSuccess) return err;
+  return cudaFuncSetAttribute(pml_kernel<DIM, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
+}
+
+template <int DIM, int N>
+static cudaError_t launch_stage_one(const StageArgs& a, int num_sms, cudaStream_t s) {
+  using C = StageCfg<DIM, N>;
+  int64_t nbatch = (a.K + C::EB - 1) / C::EB;
+  if (nbatch == 0) return cudaSuccess;
+  int per_sm = (int)(200 * 1024 / C::smem_bytes);
+  if (per_sm < 1) per_sm = 1;
+  if (per_sm > 2048 / C::Threads) per_sm = 2048 / C::Threads;
+  int64_t grid = (int64_t)num_sms * per_sm;
+  if (grid > nbatch) grid = nbatch;
+  stage_kernel<DIM, N><<<(int)grid, C::Threads, C::smem_bytes, s>>>(a);
+  return cudaGetLastError();
+}
+
+template <int DIM, int N>
+static cudaError_t launch_pml_one(const PmlArgs& a, int num_sms, cudaStream_t s) {
+  using C = StageCfg<DIM, N>;
+  int64_t nbatch = (a.Kpml + C::EB - 1) / C::EB;
+  if (nbatch == 0) return cudaSuccess;
+  int per_sm = (int)(200 * 1024 / C::smem_bytes);
+  if (per_sm < 1) per_sm = 1;
+  if (per_sm > 2048 / C::Threads) per_sm = 2048 / C::Threads;
+  int64_t grid = (int64_t)num_sms * per_sm;
+  if (grid > nbatch) grid = nbatch;
+  pml_kernel<DIM, N><<<(int)grid, C::Threads, C::smem_bytes, s>>>(a);
+  return cudaGetLastError();
+}
+
+#define ALEGB_DISPATCH(FN, ...)                                          \
+  switch (dim * 10 + N) {                                                \
+    case 21: return FN<2, 1>(__VA_ARGS__);                               \
+    case 22: return FN<2, 2>(__VA_ARGS__);                               \
+    case 23: return FN<2, 3>(__VA_ARGS__);                               \
+    case 24: return FN<2, 4>(__VA_ARGS__);                               \
+    case 25: return FN<2, 5>(__VA_ARGS__);                               \
+    case 31: return FN<3, 1>(__VA_ARGS__);                               \
+    case 32: return FN<3, 2>(__VA_ARGS__);                               \
+    case 33: return FN<3, 3>(__VA_ARGS__);                               \
+    case 34: return FN<3, 4>(__VA_ARGS__);                               \
+    case 35: return FN<3, 5>(__VA_ARGS__);                               \
+    default: return cudaErrorInvalidValue;                               \
+  }
+
+cudaError_t configure_kernels(int dim, int N) { ALEGB_DISPATCH(configure_one) }
+cudaError_t launch_stage(int dim, int N, const StageArgs& a, int num_sms, cudaStream_t s) {
+  ALEGB_DISPATCH(launch_stage_one, a, num_sms, s)
+}
+cudaError_t launch_pml(int dim, int N, const PmlArgs& a, int num_sms, cudaStream_t s) {
+  ALEGB_DISPATCH(launch_pml_one, a, num_sms, s)
+}
+
+}  // namespace alegb
