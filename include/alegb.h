@@ -21,7 +21,8 @@
  *   - "DEVICE" pointers are owned by the caller (e.g. torch tensors), must be 16-byte aligned and valid on the
  *     context's device; the library never frees or retains them beyond the enqueued work.
  *   - compute calls enqueue on the given stream (a cudaStream_t passed as void*, NULL = default stream) and do NOT
- *     synchronise.  alegb_mesh_upload, alegb_get_* and alegb_destroy synchronise the device.
+ *     synchronise.  A context owns one step workspace (stage states, geometry): calls on the same context from
+ *     different streams must be ordered by the caller.  alegb_mesh_upload, alegb_get_* and alegb_destroy synchronise the device.
  *   - field layout: q[K][Nf][Np] (element, field, node), node fastest.  Nf = 6 (2-D) or 10 (3-D), field order
  *     2-D (a00,a10,a01,a11,a20,a02) = the paper's q1..q6 (L43-51);
  *     3-D (a000; a100,a010,a001; a110,a101,a011; a200,a020,a002)   (reading R3).
@@ -145,6 +146,11 @@ int64_t alegb_workspace_bytes(const alegb_ctx* ctx);
 const char* alegb_last_error(const alegb_ctx* ctx);
 /* number of kernel launches the library has enqueued on this context since creation */
 int64_t alegb_launch_count(const alegb_ctx* ctx);
+/* Stage-kernel timing for roofline reports: while enabled, every launch of the fused stage kernel is bracketed by
+ * CUDA events on its stream (at most 4096 launches are kept per enable).  alegb_profile_read synchronises the
+ * device and returns the number of bracketed launches and the sum of their durations in milliseconds. */
+int alegb_profile_enable(alegb_ctx* ctx, int on);
+int alegb_profile_read(alegb_ctx* ctx, int64_t* launches, double* total_ms);
 /* Synchronous convenience entry for host buffers (HOST q [K][Nf][Np], updated in place): copies q to the device,
  * runs nsteps SARK4 steps, copies the result back, synchronises.  Used for end-to-end timing. */
 int alegb_step_host(alegb_ctx* ctx, double* h_q, double t0, double dt, int nsteps);

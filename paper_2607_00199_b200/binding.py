@@ -48,6 +48,8 @@ _SIGNATURES = {
     "alegb_workspace_bytes": (_c.c_int64, [_P]),
     "alegb_last_error": (_c.c_char_p, [_P]),
     "alegb_launch_count": (_c.c_int64, [_P]),
+    "alegb_profile_enable": (_c.c_int, [_P, _c.c_int]),
+    "alegb_profile_read": (_c.c_int, [_P, _c.POINTER(_c.c_int64), _c.POINTER(_c.c_double)]),
 }
 for _name, (_res, _args) in _SIGNATURES.items():
     _fn = getattr(_lib, _name)          # AttributeError here = the library does not export a declared symbol
@@ -212,6 +214,14 @@ class Context:
 
     def alegb_launch_count(self):
         return int(_lib.alegb_launch_count(self._h))
+
+    def alegb_profile_enable(self, on):
+        self._check(_lib.alegb_profile_enable(self._h, int(bool(on))))
+
+    def alegb_profile_read(self):
+        n, ms = _c.c_int64(), _c.c_double()
+        self._check(_lib.alegb_profile_read(self._h, ctypes.byref(n), ctypes.byref(ms)))
+        return int(n.value), float(ms.value)
 
     def alegb_last_error(self):
         return (_lib.alegb_last_error(self._h) or b"").decode()

@@ -36,6 +36,9 @@ struct alegb_ctx {
   double *d_AUX = nullptr, *d_AUXS = nullptr, *d_AUXACC = nullptr;
   int64_t workspace_bytes = 0;
   int64_t launches = 0;
+  bool profiling = false;
+  std::vector<cudaEvent_t> prof_events;  // pairs (start, stop), created on demand
+  size_t prof_used = 0;
   std::string err;
 };
 
@@ -128,6 +131,26 @@ int check_ready(alegb_ctx* ctx) {
   return ALEGB_OK;
 }
 
+// the fused stage kernel, bracketed by events while profiling is enabled
+int timed_stage(alegb_ctx* ctx, const StageArgs& a, cudaStream_t s) {
+  const bool rec = ctx->profiling && ctx->prof_used + 2 <= 8192;
+  if (rec) {
+    while (ctx->prof_events.size() < ctx->prof_used + 2) {
+      cudaEvent_t ev;
+      CU(cudaEventCreate(&ev));
+      ctx->prof_events.push_back(ev);
+    }
+    CU(cudaEventRecord(ctx->prof_events[ctx->prof_used], s));
+  }
+  CU(launch_stage(ctx->ref.dim, ctx->ref.N, a, ctx->num_sms, s));
+  ctx->launches++;
+  if (rec) {
+    CU(cudaEventRecord(ctx->prof_events[ctx->prof_used + 1], s));
+    ctx->prof_used += 2;
+  }
+  return ALEGB_OK;
+}
+
 // One SARK4 step.  q_n: state at t0 (read only); outs[i]: where stage state i+1 is written
 // (outs[3] = q_{n+1}, may alias q_n).
 int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t0, double dt, cudaStream_t s) {
@@ -179,8 +202,8 @@ int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t
       cf.cq_acc = 1.0;
       for (int k = 0; k < Nf; ++k) cf.cq_f[k] = dt * B(k, 3);
     }
-    CU(launch_stage(dim, N, a, ctx->num_sms, s));
-    ctx->launches++;
+    rc = timed_stage(ctx, a, s);
+    if (rc != ALEGB_OK) return rc;
     if (pml) {
       // auxiliary fields: Lambda = 0, classic RK4 weights (reading R12)
       PmlArgs p;
@@ -255,6 +278,7 @@ int alegb_destroy(alegb_ctx* ctx) {
     cudaDeviceSynchronize();
   }
   free_mesh(ctx);
+  for (cudaEvent_t ev : ctx->prof_events) cudaEventDestroy(ev);
   dev_free(ctx->d_Dt); dev_free(ctx->d_LIFTt); dev_free(ctx->d_lam); dev_free(ctx->d_fmask);
   delete ctx;
   return ALEGB_OK;
@@ -407,8 +431,8 @@ int alegb_rhs_pml(alegb_ctx* ctx, double t, const double* d_q, const double* d_a
   fill_common(ctx, a);
   a.q_in = d_q; a.F_out = d_F;
   a.aux = ctx->Kpml > 0 ? (d_aux ? d_aux : ctx->d_AUX) : nullptr;
-  CU(launch_stage(ctx->ref.dim, ctx->ref.N, a, ctx->num_sms, s));
-  ctx->launches++;
+  rc = timed_stage(ctx, a, s);
+  if (rc != ALEGB_OK) return rc;
   if (d_Faux && ctx->Kpml > 0) {
     PmlArgs p;
     fill_common(ctx, p);
@@ -563,6 +587,29 @@ int alegb_get_reference(const alegb_ctx* ctx, double* w, double* lam, int32_t* f
 int alegb_sark_coefficients(double gamma, double* a, double* b) {
   if (!a || !b) return ALEGB_INVALID_ARG;
   sark_coefficients(gamma, a, b);
+  return ALEGB_OK;
+}
+
+int alegb_profile_enable(alegb_ctx* ctx, int on) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  ctx->profiling = on != 0;
+  ctx->prof_used = 0;
+  return ALEGB_OK;
+}
+
+int alegb_profile_read(alegb_ctx* ctx, int64_t* launches, double* total_ms) {
+  if (!ctx || !launches || !total_ms) return ALEGB_INVALID_ARG;
+  if (ctx->device < 0) return fail(ctx, ALEGB_CUDA_ERROR, "host-only context (no CUDA device)");
+  CU(cudaSetDevice(ctx->device));
+  CU(cudaDeviceSynchronize());
+  double sum = 0.0;
+  for (size_t i = 0; i + 1 < ctx->prof_used; i += 2) {
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, ctx->prof_events[i], ctx->prof_events[i + 1]));
+    sum += ms;
+  }
+  *launches = (int64_t)(ctx->prof_used / 2);
+  *total_ms = sum;
   return ALEGB_OK;
 }
 

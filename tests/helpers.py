@@ -12,3 +12,31 @@ def oracle_problem(cfg, ref):
 def rel_linf(a, b):
     """DESIGN.md R15: max |a-b| over everything, divided by max |b| over the whole state."""
     return float(np.abs(a - b).max() / np.abs(b).max())
+
+
+def submesh(cfg, EToE, samples, rings):
+    """Workload dict restricted to ``samples`` plus ``rings`` layers of face neighbours (EToE from the oracle's
+    connectivity).  Faces whose neighbour is outside the patch become far-field faces (tag 2), so the operator on
+    the patch equals the full operator wherever the stencil stays inside: F on the samples needs 1 ring, stage
+    state i of one SARK step needs i rings.  Returns (sub_cfg, patch_element_ids, position_of_samples_in_patch)."""
+    samples = np.asarray(samples, dtype=np.int64)
+    patch = np.unique(samples)
+    for _ in range(rings):
+        patch = np.unique(np.concatenate([patch, EToE[patch].ravel()]))
+    inside = np.zeros(EToE.shape[0], dtype=bool)
+    inside[patch] = True
+    tags = np.where(inside[EToE[patch]], 0, 2).astype(np.int8)
+    if cfg.get("EToB") is not None:
+        orig = np.asarray(cfg["EToB"])[patch]
+        tags = np.where(orig != 0, orig, tags).astype(np.int8)
+    sub = dict(cfg)
+    sub["EToV"] = np.ascontiguousarray(cfg["EToV"][patch])
+    sub["EToB"] = tags
+    sub["K"] = len(patch)
+    if cfg.get("pml_sigma") is not None:
+        sub["pml_sigma"] = np.ascontiguousarray(np.asarray(cfg["pml_sigma"])[patch])
+    if cfg.get("q_inf") is None:
+        sub["q_inf"] = np.zeros(cfg["Nf"])
+    sub["q0"] = np.ascontiguousarray(cfg["q0"][patch])
+    where = np.searchsorted(patch, samples)
+    return sub, patch, where

@@ -1,0 +1,359 @@
+"""Parity of the CUDA path (through the C-ABI) with the CPU oracle, element by element, on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star; R15):
+  stage states   max|q_gpu - q_orc| / max|q_orc| <= 1e-12 per stage, <= 1e-10 after 100 steps
+  F(q, t)        |F_gpu - F_orc| <= 1e-12 * Fabs pointwise, Fabs = the oracle's sum of absolute values of all terms
+  geometry       relative 1e-13
+Everything here needs a GPU (-m gpu) and calls the library only through paper_2607_00199_b200.binding.
+"""
+import numpy as np
+import pytest
+
+from oracle import mesh as omesh
+from oracle import motion as omotion
+from oracle import physics, sark
+from workloads import configs, meshes
+from helpers import oracle_problem, rel_linf, submesh
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL_STAGE, TOL_100, TOL_F = 1e-12, 1e-10, 1e-12
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu tests must run on the B200 box")
+    from paper_2607_00199_b200 import binding
+    return binding
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def perturbed(cfg, amp=1e-3, seed=7):
+    """Initial state with seeded element-wise noise, so that every face carries a jump."""
+    rng = np.random.default_rng(seed)
+    return cfg["q0"] * (1.0 + amp * rng.standard_normal(cfg["q0"].shape))
+
+
+def swimmer_small(lam, n=(12, 6, 6), lo=(-4.0, -3.0, -3.0), hi=(8.0, 3.0, 3.0)):
+    """config 5 shape with a body fat enough to be resolved by a coarse grid (wall faces, far field, PML)."""
+    cfg = configs.config5(lam, nx=n[0], ny=n[1], nz=n[2])
+    X0, EToV, EToB, sigma = meshes.swimmer_box(n[0], n[1], n[2], half_height=1.2, half_width=1.2,
+                                               lo=lo, hi=hi)
+    cfg.update(X0=X0, EToV=EToV, EToB=EToB, pml_sigma=sigma)
+    cfg["motion_params"] = cfg["motion_params"].copy()
+    cfg["motion_params"][5] = 2.0                   # R_rigid: make the layer around the body move
+    cfg["dt"] = configs.cfl_dt(3, 3, X0, EToV, cfg["RT"], 0.5, 0.2 * cfg["motion_params"][4])
+    return configs._finish(cfg, lam)
+
+
+def make_case(name, refs):
+    if name == "cfg1":
+        ref = refs(2, 3); cfg = configs.config1(ref.lam)
+    elif name == "cfg2":
+        ref = refs(2, 4); cfg = configs.config2(ref.lam, n=12)
+    elif name == "cfg3":
+        ref = refs(2, 4); cfg = configs.config3(ref.lam, ntheta=24, nr=10)
+    elif name == "cfg4":
+        ref = refs(3, 4); cfg = configs.config4(ref.lam, n=4)
+    elif name == "cfg5":
+        ref = refs(3, 3); cfg = swimmer_small(ref.lam)
+    elif name == "cfg5_tiny":
+        ref = refs(3, 3); cfg = swimmer_small(ref.lam, n=(8, 4, 4), lo=(-2.0, -1.5, -1.5), hi=(4.0, 1.5, 1.5))
+    elif name == "tri_N1":
+        ref = refs(2, 1); cfg = configs.config2(ref.lam, n=7); cfg["N"] = 1; cfg = configs._finish(cfg, ref.lam)
+    elif name == "tri_N5":
+        ref = refs(2, 5); cfg = configs.config2(ref.lam, n=5); cfg["N"] = 5; cfg = configs._finish(cfg, ref.lam)
+    elif name == "tet_N2":
+        ref = refs(3, 2); cfg = configs.config4(ref.lam, n=3); cfg["N"] = 2; cfg = configs._finish(cfg, ref.lam)
+    elif name == "tet_N5":
+        ref = refs(3, 5); cfg = configs.config4(ref.lam, n=3); cfg["N"] = 5; cfg = configs._finish(cfg, ref.lam)
+    else:
+        raise KeyError(name)
+    return ref, cfg
+
+
+CASES = ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "tri_N1", "tri_N5", "tet_N2", "tet_N5"]
+
+
+@pytest.mark.parametrize("name", CASES)
+def test_geometry_matches_oracle(name, refs, B):
+    ref, cfg = make_case(name, refs)
+    P = oracle_problem(cfg, ref)
+    ctx = B.context_from_config(cfg)
+    dim, K = cfg["dim"], cfg["K"]
+    for t in (0.0, 0.137, 0.77):
+        vgeo = torch.empty(K, dim * dim + 1, dtype=torch.float64, device="cuda")
+        sgeo = torch.empty(K, dim + 1, dim + 2, dtype=torch.float64, device="cuda")
+        xv = torch.empty(cfg["X0"].shape, dtype=torch.float64, device="cuda")
+        vv = torch.empty_like(xv)
+        ctx.alegb_geometry(t, vgeo, sgeo, xv, vv)
+        torch.cuda.synchronize()
+        g = P.geometry(t)
+        vgeo, sgeo = vgeo.cpu().numpy(), sgeo.cpu().numpy()
+        assert np.abs(xv.cpu().numpy() - g["xv"]).max() <= 1e-14 * np.abs(g["xv"]).max()
+        assert np.abs(vv.cpu().numpy() - g["vv"]).max() <= 1e-13 * max(np.abs(g["vv"]).max(), 1e-300)
+        assert rel_linf(vgeo[:, -1], g["J"]) < 1e-13
+        assert rel_linf(vgeo[:, :-1].reshape(K, dim, dim), g["Ginv"]) < 1e-13
+        assert np.abs(sgeo[:, :, :dim] - g["nhat"]).max() < 1e-13
+        assert rel_linf(sgeo[:, :, dim], g["sJ"]) < 1e-13
+        assert rel_linf(sgeo[:, :, dim + 1], g["Fscale"]) < 1e-13
+    ctx.close()
+
+
+@pytest.mark.parametrize("name", CASES)
+def test_rhs_matches_oracle(name, refs, B):
+    ref, cfg = make_case(name, refs)
+    P = oracle_problem(cfg, ref)
+    ctx = B.context_from_config(cfg)
+    q = perturbed(cfg)
+    dq, dF = dev(q), torch.empty(q.shape, dtype=torch.float64, device="cuda")
+    for t in (0.0, 0.31):
+        if P.sigma is None:
+            ctx.alegb_rhs(t, dq, dF)
+            torch.cuda.synchronize()
+            F, Fabs = P.rhs(q, t, want_abs=True)
+        else:
+            rng = np.random.default_rng(11)
+            aux = 1e-3 * rng.standard_normal((len(P.pml_elems), cfg["dim"]) + q.shape[1:])
+            daux, dG = dev(aux), torch.empty(aux.shape, dtype=torch.float64, device="cuda")
+            ctx.alegb_rhs_pml(t, dq, daux, dF, dG)
+            torch.cuda.synchronize()
+            F, G, Fabs = P.rhs(q, t, aux=aux, want_abs=True)
+            assert np.array_equal(ctx.alegb_pml_elements(), P.pml_elems)
+            # the auxiliary right-hand side has no Fabs of its own: its terms are a subset of F's
+            assert np.abs(dG.cpu().numpy() - G).max() <= TOL_F * (Fabs[P.pml_elems].max() + np.abs(G).max())
+        err = np.abs(dF.cpu().numpy() - F)
+        floor = 1e-3 * Fabs.max()
+        assert (err <= TOL_F * (Fabs + floor)).all(), (err / (Fabs + floor)).max()
+        assert err.max() <= 1e-12 * np.abs(F).max()
+    ctx.close()
+
+
+@pytest.mark.parametrize("name", CASES)
+def test_stage_states_match_oracle(name, refs, B):
+    """R19: the four stage states of one step, at step 1 and (cfg1, cfg2, cfg4) again at step 100."""
+    ref, cfg = make_case(name, refs)
+    P = oracle_problem(cfg, ref)
+    ctx = B.context_from_config(cfg)
+    q = perturbed(cfg)
+    dt = cfg["dt"]
+    st = torch.empty((4,) + q.shape, dtype=torch.float64, device="cuda")
+    ctx.alegb_step_debug(dev(q), 0.05, dt, st)
+    torch.cuda.synchronize()
+    so, aux = sark.step_debug(P, q, 0.05, dt)
+    for i in range(4):
+        assert rel_linf(st[i].cpu().numpy(), so[i]) <= TOL_STAGE
+    if aux is not None:
+        da = torch.empty(aux.shape, dtype=torch.float64, device="cuda")
+        ctx.alegb_pml_get(da)
+        torch.cuda.synchronize()
+        assert np.abs(da.cpu().numpy() - aux).max() <= TOL_STAGE * max(np.abs(aux).max(), np.abs(q).max() * 1e-6)
+    ctx.close()
+
+
+@pytest.mark.parametrize("name,nsteps", [("cfg1", 100), ("cfg2", 100), ("cfg3", 100), ("cfg4", 100), ("cfg5_tiny", 100)])
+def test_hundred_steps_match_oracle(name, nsteps, refs, B):
+    ref, cfg = make_case(name, refs)
+    P = oracle_problem(cfg, ref)
+    ctx = B.context_from_config(cfg)
+    q = perturbed(cfg, amp=1e-4)
+    dt = cfg["dt"]
+    dq = dev(q)
+    ctx.alegb_step(dq, 0.0, dt, nsteps - 1)
+    torch.cuda.synchronize()
+    out = sark.step(P, q, 0.0, dt, nsteps - 1)
+    qo, aux = out if isinstance(out, tuple) else (out, None)
+    assert rel_linf(dq.cpu().numpy(), qo) <= TOL_100
+    # stage states of step number `nsteps`, each side continuing from its own state
+    st = torch.empty((4,) + q.shape, dtype=torch.float64, device="cuda")
+    ctx.alegb_step_debug(dq, (nsteps - 1) * dt, dt, st)
+    torch.cuda.synchronize()
+    so, _ = sark.step_debug(P, qo, (nsteps - 1) * dt, dt, aux)
+    for i in range(4):
+        assert rel_linf(st[i].cpu().numpy(), so[i]) <= TOL_100
+    ctx.close()
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_free_stream_preserved_on_gpu(dim, refs, B):
+    """GCL (Table 2): a uniform state stays uniform on the deforming mesh, every stage."""
+    if dim == 2:
+        ref = refs(2, 3); cfg = configs.config1(ref.lam); nsteps = 50
+    else:
+        ref = refs(3, 4); cfg = configs.config4(ref.lam, n=6); nsteps = 20
+        u = np.broadcast_to([0.1, 0.05, -0.02], (cfg["K"], ref.Np, 3))
+        cfg["q0"] = np.ascontiguousarray(np.transpose(configs.maxwellian(3, np.ones((cfg["K"], ref.Np)), u, 1.0), (0, 2, 1)))
+    ctx = B.context_from_config(cfg)
+    q0 = cfg["q0"]
+    st = torch.empty((4,) + q0.shape, dtype=torch.float64, device="cuda")
+    ctx.alegb_step_debug(dev(q0), 0.13, cfg["dt"], st)
+    torch.cuda.synchronize()
+    assert np.abs(st.cpu().numpy() - q0[None]).max() < 1e-14
+    dq = dev(q0)
+    ctx.alegb_step(dq, 0.0, cfg["dt"], nsteps)
+    torch.cuda.synchronize()
+    assert np.abs(dq.cpu().numpy() - q0).max() < 1e-13
+    xv = torch.empty(cfg["X0"].shape, dtype=torch.float64, device="cuda")
+    ctx.alegb_geometry(0.25, d_xv=xv)
+    torch.cuda.synchronize()
+    assert np.abs(xv.cpu().numpy() - cfg["X0"]).max() > 0.02      # the mesh really moved
+    ctx.close()
+
+
+def test_uniform_relaxation_exact_on_gpu(refs, B):
+    """R8 pin on the device: uniform non-equilibrium state, q4(t) = q4eq + (q4(0)-q4eq) e^{-t/tau} to round-off."""
+    ref = refs(2, 3)
+    cfg = configs.config1(ref.lam, n=4)
+    ctx = B.context_from_config(cfg)
+    qe = physics.equilibrium_state(2, np.array(1.0), np.array([0.1, 0.05]), 1.0)
+    q0 = qe.copy(); q0[3:] += np.array([0.02, -0.01, 0.03])
+    q = np.broadcast_to(q0[None, :, None], (cfg["K"], 6, ref.Np)).copy()
+    dt, n = 0.4 * cfg["tau"], 25
+    dq = dev(q)
+    ctx.alegb_step(dq, 0.0, dt, n)
+    torch.cuda.synchronize()
+    exact = qe + (q0 - qe) * np.exp(-n * dt / cfg["tau"] * physics.stiff_mask(2))
+    assert np.abs(dq.cpu().numpy() - exact[None, :, None]).max() < 5e-15
+    ctx.close()
+
+
+def test_collisionless_and_static(refs, B):
+    """tau = inf (classic RK4, no relaxation) and no motion: both degenerate branches against the oracle."""
+    ref = refs(2, 3)
+    cfg = configs.config1(ref.lam, n=5)
+    cfg["tau"] = float("inf"); cfg["motion_kind"] = 0; cfg["motion_params"] = None
+    P = oracle_problem(cfg, ref)
+    ctx = B.context_from_config(cfg)
+    q = perturbed(cfg)
+    st = torch.empty((4,) + q.shape, dtype=torch.float64, device="cuda")
+    ctx.alegb_step_debug(dev(q), 0.0, cfg["dt"], st)
+    torch.cuda.synchronize()
+    so, _ = sark.step_debug(P, q, 0.0, cfg["dt"])
+    for i in range(4):
+        assert rel_linf(st[i].cpu().numpy(), so[i]) <= TOL_STAGE
+    ctx.close()
+
+
+def test_user_motion_equals_builtin(refs, B):
+    ref, cfg = make_case("cfg4", refs)
+    P = oracle_problem(cfg, ref)
+    t = 0.21
+    xv, vv = omotion.vertices(cfg["motion_kind"], cfg["motion_params"], cfg["X0"], t)
+    ctx = B.context_from_config(cfg)
+    q = perturbed(cfg)
+    dq, dF = dev(q), torch.empty(q.shape, dtype=torch.float64, device="cuda")
+    ctx.alegb_set_motion_user(dev(xv), dev(vv))
+    ctx.alegb_rhs(123.0, dq, dF)                      # time is irrelevant for USER motion
+    torch.cuda.synchronize()
+    F, Fabs = P.rhs(q, t, want_abs=True)
+    assert (np.abs(dF.cpu().numpy() - F) <= TOL_F * (Fabs + 1e-3 * Fabs.max())).all()
+    ctx.close()
+
+
+def test_single_element_and_ragged_batches(refs, B):
+    """K = 1 (every face a far-field face) and K values around the kernel's batch sizes."""
+    ref = refs(3, 3)
+    X0 = np.array([[0, 0, 0], [1, 0, 0], [0, 1, 0], [0, 0, 1.0]])
+    q_inf = physics.equilibrium_state(3, np.array(1.0), np.array([0.1, 0.0, 0.05]), 1.0)
+    for K in (1, 2, 11, 13, 25):
+        XX = np.concatenate([X0 + np.array([3.0 * k, 0, 0]) for k in range(K)])
+        EToV = np.arange(4 * K, dtype=np.int32).reshape(K, 4)
+        EToB = np.full((K, 4), 2, dtype=np.int8)
+        cfg = dict(dim=3, N=3, X0=XX, EToV=EToV, vertex_equiv=None, EToB=EToB, pml_sigma=None, RT=1.0, tau=1e-2,
+                   q_inf=q_inf, motion_kind=2, motion_params=np.array([0.02, 1.0, 2.0, 0.3]), K=K, Np=20, Nf=10)
+        rng = np.random.default_rng(K)
+        q = q_inf[None, :, None] * (1.0 + 1e-2 * rng.standard_normal((K, 10, 20)))
+        P = oracle_problem(cfg, ref)
+        ctx = B.context_from_config(cfg)
+        st = torch.empty((4,) + q.shape, dtype=torch.float64, device="cuda")
+        ctx.alegb_step_debug(dev(q), 0.1, 1e-3, st)
+        torch.cuda.synchronize()
+        so, _ = sark.step_debug(P, q, 0.1, 1e-3)
+        for i in range(4):
+            assert rel_linf(st[i].cpu().numpy(), so[i]) <= TOL_STAGE
+        ctx.close()
+
+
+def test_streams_alignment_and_errors(refs, B):
+    ref, cfg = make_case("cfg1", refs)
+    ctx = B.context_from_config(cfg)
+    q = perturbed(cfg)
+    s = torch.cuda.Stream()
+    dq = dev(q)
+    a, b = dq.clone(), dq.clone()
+    torch.cuda.synchronize()
+    ctx.alegb_step(a, 0.0, cfg["dt"], 3)
+    torch.cuda.synchronize()          # one context = one workspace: calls on different streams must not overlap
+    with torch.cuda.stream(s):
+        ctx.alegb_step(b, 0.0, cfg["dt"], 3, stream=s)
+    torch.cuda.synchronize()
+    assert torch.equal(a, b)                              # same kernels, same order: bit-identical
+    n0 = ctx.alegb_launch_count()
+    ctx.alegb_step(a, 0.0, cfg["dt"], 2)
+    assert ctx.alegb_launch_count() - n0 >= 2 * 4         # at least one launch per stage
+    buf = torch.empty(q.size + 1, dtype=torch.float64, device="cuda")
+    with pytest.raises(B.AlegbError) as e:
+        ctx.alegb_step(buf.data_ptr() + 8, 0.0, cfg["dt"], 1)
+    assert e.value.status == B.INVALID_ARG
+    fresh = B.Context(2, 3, 0)
+    with pytest.raises(B.AlegbError) as e:
+        fresh.alegb_rhs(0.0, dq, a)
+    assert e.value.status == B.NOT_READY
+    fresh.close(); ctx.close()
+
+
+def test_step_host_roundtrip(refs, B):
+    ref, cfg = make_case("cfg2", refs)
+    ctx = B.context_from_config(cfg)
+    q = perturbed(cfg)
+    dq = dev(q)
+    ctx.alegb_step(dq, 0.0, cfg["dt"], 2)
+    hq = torch.from_numpy(q.copy()).pin_memory()
+    ctx.alegb_step_host(hq, 0.0, cfg["dt"], 2)
+    assert np.array_equal(hq.numpy(), dq.cpu().numpy())
+    ctx.close()
+
+
+def test_full_size_throughput_config_sampled(refs, B):
+    """BASELINE.json configs[3] at full size (196,608 tets, N = 4), the launch configuration bench.py times.
+    The oracle computes a sample of elements one patch at a time (helpers.submesh): F needs the face neighbours,
+    stage state i needs i rings of them."""
+    ref = refs(3, 4)
+    cfg = configs.config4(ref.lam)
+    assert cfg["K"] == 196608
+    conn = omesh.connect(ref, cfg["EToV"], cfg["vertex_equiv"])
+    ctx = B.context_from_config(cfg)
+    q = perturbed(cfg, amp=1e-4)
+    cfg["q0"] = q
+    dq = dev(q)
+    dF = torch.empty_like(dq)
+    t, dt = 0.2, cfg["dt"]
+    ctx.alegb_rhs(t, dq, dF)
+    st = torch.empty((4,) + q.shape, dtype=torch.float64, device="cuda")
+    ctx.alegb_step_debug(dq, t, dt, st)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(5)
+    samples = np.concatenate([[0, 1, cfg["K"] - 1, cfg["K"] - 2], rng.integers(0, cfg["K"], size=8)])
+    Fg = dF[torch.from_numpy(samples).cuda()].cpu().numpy()
+    sub, patch, where = submesh(cfg, conn["EToE"], samples, rings=1)
+    F, Fabs = oracle_problem(sub, ref).rhs(sub["q0"], t, want_abs=True)
+    assert (np.abs(Fg - F[where]) <= TOL_F * (Fabs[where] + 1e-3 * Fabs.max())).all()
+    for s0 in samples[:6]:
+        sub, patch, where = submesh(cfg, conn["EToE"], [s0], rings=4)
+        so, _ = sark.step_debug(oracle_problem(sub, ref), sub["q0"], t, dt)
+        for i in range(4):
+            got = st[i, int(s0)].cpu().numpy()
+            assert np.abs(got - so[i][where[0]]).max() <= TOL_STAGE * np.abs(so[i]).max()
+    # property that holds at any size: the uniform state is a fixed point of the step on the deforming mesh
+    u = np.broadcast_to([0.1, 0.05, -0.02], (cfg["K"], ref.Np, 3))
+    q0 = np.ascontiguousarray(np.transpose(configs.maxwellian(3, np.ones((cfg["K"], ref.Np)), u, 1.0), (0, 2, 1)))
+    dq = dev(q0)
+    ctx.alegb_step(dq, 0.0, dt, 3)
+    torch.cuda.synchronize()
+    assert np.abs(dq.cpu().numpy() - q0).max() < 1e-13
+    ctx.close()

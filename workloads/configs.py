@@ -13,7 +13,7 @@ import numpy as np
 from . import meshes
 
 SEED = 199
-NP_OF = {(2, 1): 3, (2, 2): 6, (2, 3): 10, (2, 4): 15, (3, 1): 4, (3, 2): 10, (3, 3): 20, (3, 4): 35}
+NP_OF = {(2, 1): 3, (2, 2): 6, (2, 3): 10, (2, 4): 15, (2, 5): 21, (3, 1): 4, (3, 2): 10, (3, 3): 20, (3, 4): 35, (3, 5): 56}
 NF_OF = {2: 6, 3: 10}
 FACE_VERTS = {2: [[0, 1], [1, 2], [2, 0]], 3: [[0, 1, 2], [0, 1, 3], [1, 2, 3], [0, 2, 3]]}
 
