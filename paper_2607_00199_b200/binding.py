@@ -48,6 +48,7 @@ _SIGNATURES = {
     "alegb_workspace_bytes": (_c.c_int64, [_P]),
     "alegb_last_error": (_c.c_char_p, [_P]),
     "alegb_launch_count": (_c.c_int64, [_P]),
+    "alegb_set_kernel": (_c.c_int, [_P, _c.c_int]),
     "alegb_profile_enable": (_c.c_int, [_P, _c.c_int]),
     "alegb_profile_read": (_c.c_int, [_P, _c.POINTER(_c.c_int64), _c.POINTER(_c.c_double)]),
 }
@@ -214,6 +215,9 @@ class Context:
 
     def alegb_launch_count(self):
         return int(_lib.alegb_launch_count(self._h))
+
+    def alegb_set_kernel(self, kind):
+        self._check(_lib.alegb_set_kernel(self._h, int(kind)))
 
     def alegb_profile_enable(self, on):
         self._check(_lib.alegb_profile_enable(self._h, int(bool(on))))

@@ -22,8 +22,10 @@ struct alegb_ctx {
   MotionArgs motion{};
   std::vector<int32_t> vmapM_host, vmapP_host, pml_elems_host;
   // device: operators
-  double *d_Dt = nullptr, *d_LIFTt = nullptr, *d_lam = nullptr;
+  double *d_Dt = nullptr, *d_LIFTt = nullptr, *d_lam = nullptr, *d_Avol = nullptr, *d_Alift = nullptr;
   int32_t* d_fmask = nullptr;
+  bool mma_ok = false;   // a DMMA stage kernel exists for (dim, N)
+  int kernel_mode = 0;   // 0 auto (DMMA where available), 1 generic, 2 DMMA
   // device: mesh
   double *d_X0 = nullptr, *d_xv = nullptr, *d_vv = nullptr;
   int32_t *d_EToV = nullptr, *d_vmapP = nullptr;
@@ -108,6 +110,7 @@ void fill_common(const alegb_ctx* ctx, StageArgs& a) {
   a.vmapP = ctx->d_vmapP; a.EToB = ctx->d_EToB;
   a.pml_index = ctx->d_pml_index; a.pml_sigma = ctx->d_pml_sigma;
   a.Dt_ops = ctx->d_Dt; a.LIFTt = ctx->d_LIFTt; a.lam = ctx->d_lam; a.fmask = ctx->d_fmask;
+  a.Avol = ctx->d_Avol; a.Alift = ctx->d_Alift;
   a.c = ctx->c; a.invtau = ctx->invtau;
   for (int k = 0; k < kMaxFields; ++k) a.q_inf[k] = ctx->q_inf[k];
 }
@@ -142,7 +145,8 @@ int timed_stage(alegb_ctx* ctx, const StageArgs& a, cudaStream_t s) {
     }
     CU(cudaEventRecord(ctx->prof_events[ctx->prof_used], s));
   }
-  CU(launch_stage(ctx->ref.dim, ctx->ref.N, a, ctx->num_sms, s));
+  if (ctx->mma_ok && ctx->kernel_mode != 1) CU(launch_stage_mma(ctx->ref.dim, ctx->ref.N, a, ctx->num_sms, s));
+  else CU(launch_stage(ctx->ref.dim, ctx->ref.N, a, ctx->num_sms, s));
   ctx->launches++;
   if (rec) {
     CU(cudaEventRecord(ctx->prof_events[ctx->prof_used + 1], s));
@@ -260,6 +264,31 @@ int alegb_create(alegb_ctx** out, int dim, int N, int cuda_device) {
   for (int i = 0; i < Np; ++i)
     for (int m = 0; m < ncol; ++m) Lt[(size_t)m * Np + i] = r.LIFT[i * ncol + m];
   std::vector<int32_t> fm(r.fmask.begin(), r.fmask.end());
+  // operators in DMMA fragment order: lane l of fragment (row tile nb, k-step ks) holds A[8 nb + l/4][4 ks + l%4]
+  MmaLayout L{};
+  ctx->mma_ok = mma_layout(dim, N, L) && configure_stage_mma(dim, N) == cudaSuccess;
+  if (ctx->mma_ok) {
+    std::vector<double> Av((size_t)dim * L.NB * L.KS * 32, 0.0), Al((size_t)r.Nfaces * L.NB * L.KF * 32, 0.0);
+    for (int a = 0; a < dim; ++a)
+      for (int nb = 0; nb < L.NB; ++nb)
+        for (int ks = 0; ks < L.KS; ++ks)
+          for (int l = 0; l < 32; ++l) {
+            const int row = 8 * nb + l / 4, col = 4 * ks + l % 4;
+            if (row < Np && col < Np) Av[(((size_t)a * L.NB + nb) * L.KS + ks) * 32 + l] = r.D[a][row * Np + col];
+          }
+    for (int f = 0; f < r.Nfaces; ++f)
+      for (int nb = 0; nb < L.NB; ++nb)
+        for (int ks = 0; ks < L.KF; ++ks)
+          for (int l = 0; l < 32; ++l) {
+            const int row = 8 * nb + l / 4, m = 4 * ks + l % 4;
+            if (row < Np && m < r.Nfp) Al[(((size_t)f * L.NB + nb) * L.KF + ks) * 32 + l] = r.LIFT[row * ncol + f * r.Nfp + m];
+          }
+    if (upload(ctx, &ctx->d_Avol, Av.data(), Av.size()) != cudaSuccess ||
+        upload(ctx, &ctx->d_Alift, Al.data(), Al.size()) != cudaSuccess) {
+      alegb_destroy(ctx);
+      return ALEGB_CUDA_ERROR;
+    }
+  }
   if (upload(ctx, &ctx->d_Dt, Dt.data(), Dt.size()) != cudaSuccess ||
       upload(ctx, &ctx->d_LIFTt, Lt.data(), Lt.size()) != cudaSuccess ||
       upload(ctx, &ctx->d_lam, r.lam.data(), r.lam.size()) != cudaSuccess ||
@@ -280,6 +309,7 @@ int alegb_destroy(alegb_ctx* ctx) {
   free_mesh(ctx);
   for (cudaEvent_t ev : ctx->prof_events) cudaEventDestroy(ev);
   dev_free(ctx->d_Dt); dev_free(ctx->d_LIFTt); dev_free(ctx->d_lam); dev_free(ctx->d_fmask);
+  dev_free(ctx->d_Avol); dev_free(ctx->d_Alift);
   delete ctx;
   return ALEGB_OK;
 }
@@ -587,6 +617,14 @@ int alegb_get_reference(const alegb_ctx* ctx, double* w, double* lam, int32_t* f
 int alegb_sark_coefficients(double gamma, double* a, double* b) {
   if (!a || !b) return ALEGB_INVALID_ARG;
   sark_coefficients(gamma, a, b);
+  return ALEGB_OK;
+}
+
+int alegb_set_kernel(alegb_ctx* ctx, int kind) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  if (kind < 0 || kind > 2) return fail(ctx, ALEGB_INVALID_ARG, "kernel kind must be 0 (auto), 1 (generic) or 2 (DMMA)");
+  if (kind == 2 && !ctx->mma_ok) return fail(ctx, ALEGB_UNSUPPORTED, "no DMMA stage kernel for this (dim, N)");
+  ctx->kernel_mode = kind;
   return ALEGB_OK;
 }
 

@@ -39,6 +39,8 @@ struct StageArgs {
   const double* LIFTt;   // [Nfaces*Nfp(m)][Np(i)] : LIFT[i][m]
   const double* lam;     // [Np][dim+1]
   const int32_t* fmask;  // [Nfaces*Nfp]
+  const double* Avol;    // DMMA path: D_a in fragment order [dim][NB][KS][32]
+  const double* Alift;   // DMMA path: LIFT in fragment order [Nfaces][NB][KF][32]
   // physics
   double c, invtau;
   double q_inf[kMaxFields];
@@ -85,5 +87,11 @@ cudaError_t launch_geometry(int dim, int64_t K, const int32_t* EToV, const doubl
 cudaError_t launch_stage(int dim, int N, const StageArgs& a, int num_sms, cudaStream_t s);
 cudaError_t launch_pml(int dim, int N, const PmlArgs& a, int num_sms, cudaStream_t s);
 cudaError_t configure_kernels(int dim, int N);
+
+// tensor-core (DMMA) stage kernel, stage_mma.cu
+struct MmaLayout { int NB, KS, KF; };               // node blocks, k-steps of the volume / per-face contraction
+bool mma_layout(int dim, int N, MmaLayout& L);       // false if (dim, N) has no DMMA kernel
+cudaError_t configure_stage_mma(int dim, int N);
+cudaError_t launch_stage_mma(int dim, int N, const StageArgs& a, int num_sms, cudaStream_t s);
 
 }  // namespace alegb

@@ -78,6 +78,18 @@ def make_case(name, refs):
 
 
 CASES = ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "tri_N1", "tri_N5", "tet_N2", "tet_N5"]
+KERNELS = [1, 2]        # alegb_set_kernel: 1 = generic DFMA stage kernel, 2 = tensor-core DMMA stage kernel
+
+
+def make_ctx(B, cfg, kernel):
+    ctx = B.context_from_config(cfg)
+    try:
+        ctx.alegb_set_kernel(kernel)
+    except B.AlegbError as e:
+        assert e.status == B.UNSUPPORTED and kernel == 2
+        ctx.close()
+        pytest.skip("no DMMA kernel for dim=%d N=%d (the generic kernel covers it)" % (cfg["dim"], cfg["N"]))
+    return ctx
 
 
 @pytest.mark.parametrize("name", CASES)
@@ -105,11 +117,12 @@ def test_geometry_matches_oracle(name, refs, B):
     ctx.close()
 
 
+@pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("name", CASES)
-def test_rhs_matches_oracle(name, refs, B):
+def test_rhs_matches_oracle(name, kernel, refs, B):
     ref, cfg = make_case(name, refs)
     P = oracle_problem(cfg, ref)
-    ctx = B.context_from_config(cfg)
+    ctx = make_ctx(B, cfg, kernel)
     q = perturbed(cfg)
     dq, dF = dev(q), torch.empty(q.shape, dtype=torch.float64, device="cuda")
     for t in (0.0, 0.31):
@@ -134,12 +147,13 @@ def test_rhs_matches_oracle(name, refs, B):
     ctx.close()
 
 
+@pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("name", CASES)
-def test_stage_states_match_oracle(name, refs, B):
-    """R19: the four stage states of one step, at step 1 and (cfg1, cfg2, cfg4) again at step 100."""
+def test_stage_states_match_oracle(name, kernel, refs, B):
+    """R19: the four stage states of one step (test_hundred_steps repeats this at step 100)."""
     ref, cfg = make_case(name, refs)
     P = oracle_problem(cfg, ref)
-    ctx = B.context_from_config(cfg)
+    ctx = make_ctx(B, cfg, kernel)
     q = perturbed(cfg)
     dt = cfg["dt"]
     st = torch.empty((4,) + q.shape, dtype=torch.float64, device="cuda")
@@ -179,8 +193,9 @@ def test_hundred_steps_match_oracle(name, nsteps, refs, B):
     ctx.close()
 
 
+@pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("dim", [2, 3])
-def test_free_stream_preserved_on_gpu(dim, refs, B):
+def test_free_stream_preserved_on_gpu(dim, kernel, refs, B):
     """GCL (Table 2): a uniform state stays uniform on the deforming mesh, every stage."""
     if dim == 2:
         ref = refs(2, 3); cfg = configs.config1(ref.lam); nsteps = 50
@@ -188,7 +203,7 @@ def test_free_stream_preserved_on_gpu(dim, refs, B):
         ref = refs(3, 4); cfg = configs.config4(ref.lam, n=6); nsteps = 20
         u = np.broadcast_to([0.1, 0.05, -0.02], (cfg["K"], ref.Np, 3))
         cfg["q0"] = np.ascontiguousarray(np.transpose(configs.maxwellian(3, np.ones((cfg["K"], ref.Np)), u, 1.0), (0, 2, 1)))
-    ctx = B.context_from_config(cfg)
+    ctx = make_ctx(B, cfg, kernel)
     q0 = cfg["q0"]
     st = torch.empty((4,) + q0.shape, dtype=torch.float64, device="cuda")
     ctx.alegb_step_debug(dev(q0), 0.13, cfg["dt"], st)
@@ -255,7 +270,8 @@ def test_user_motion_equals_builtin(refs, B):
     ctx.close()
 
 
-def test_single_element_and_ragged_batches(refs, B):
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_single_element_and_ragged_batches(kernel, refs, B):
     """K = 1 (every face a far-field face) and K values around the kernel's batch sizes."""
     ref = refs(3, 3)
     X0 = np.array([[0, 0, 0], [1, 0, 0], [0, 1, 0], [0, 0, 1.0]])
@@ -269,7 +285,7 @@ def test_single_element_and_ragged_batches(refs, B):
         rng = np.random.default_rng(K)
         q = q_inf[None, :, None] * (1.0 + 1e-2 * rng.standard_normal((K, 10, 20)))
         P = oracle_problem(cfg, ref)
-        ctx = B.context_from_config(cfg)
+        ctx = make_ctx(B, cfg, kernel)
         st = torch.empty((4,) + q.shape, dtype=torch.float64, device="cuda")
         ctx.alegb_step_debug(dev(q), 0.1, 1e-3, st)
         torch.cuda.synchronize()
