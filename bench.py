@@ -169,6 +169,8 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5],
                     help="BASELINE.json workload (1-based); 4 = the 3D N=4 throughput configuration")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--kernel", type=int, default=0, choices=[0, 1, 2, 3],
+                    help="alegb_set_kernel: 0 auto, 1 generic DFMA, 2 pipelined DMMA, 3 warp-per-quad DMMA")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -196,6 +198,7 @@ def main():
     probe.close()
     cfg = make_config(args.config, lam)
     ctx = B.context_from_config(cfg, local_rank)
+    ctx.alegb_set_kernel(args.kernel)
     K, Np, Nf, Nfp = cfg["K"], cfg["Np"], cfg["Nf"], ctx.Nfp
     dof = K * Np * Nf
     dt = cfg["dt"]
@@ -280,7 +283,7 @@ def main():
                        "dt": dt, "parallelism": "replicas x%d (north_star: one GPU, no sharding)" % world,
                        "l2": "state arrays are %.0f MB each (> 126 MB L2), no flush needed" % (state_bytes / 1e6)
                        if state_bytes > 200e6 else "state is L2-resident (%.1f MB); launch-latency bound" % (state_bytes / 1e6),
-                       "state_finite": finite},
+                       "state_finite": finite, "kernel": args.kernel},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
 
     if not args.no_cpu_baseline:

@@ -146,9 +146,10 @@ int64_t alegb_workspace_bytes(const alegb_ctx* ctx);
 const char* alegb_last_error(const alegb_ctx* ctx);
 /* number of kernel launches the library has enqueued on this context since creation */
 int64_t alegb_launch_count(const alegb_ctx* ctx);
-/* Which fused stage kernel runs: 0 = automatic (the tensor-core DMMA kernel where one is compiled for (dim, N), the
- * generic kernel otherwise), 1 = generic element-blocked DFMA kernel, 2 = DMMA kernel (ALEGB_UNSUPPORTED if there is
- * none).  Both compute the same operator; tests run both. */
+/* Which fused stage kernel runs: 0 = automatic (the pipelined tensor-core DMMA kernel where one is compiled for
+ * (dim, N), the generic kernel otherwise), 1 = generic element-blocked DFMA kernel, 2 = pipelined DMMA kernel
+ * (producer/consumer warps), 3 = warp-per-4-elements DMMA kernel; 2 and 3 return ALEGB_UNSUPPORTED if there is none.
+ * All compute the same operator; tests run all of them. */
 int alegb_set_kernel(alegb_ctx* ctx, int kind);
 /* Stage-kernel timing for roofline reports: while enabled, every launch of the fused stage kernel is bracketed by
  * CUDA events on its stream (at most 4096 launches are kept per enable).  alegb_profile_read synchronises the

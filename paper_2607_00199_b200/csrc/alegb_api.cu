@@ -24,8 +24,9 @@ struct alegb_ctx {
   // device: operators
   double *d_Dt = nullptr, *d_LIFTt = nullptr, *d_lam = nullptr, *d_Avol = nullptr, *d_Alift = nullptr;
   int32_t* d_fmask = nullptr;
-  bool mma_ok = false;   // a DMMA stage kernel exists for (dim, N)
-  int kernel_mode = 0;   // 0 auto (DMMA where available), 1 generic, 2 DMMA
+  bool mma_ok = false;   // a warp-per-quad DMMA stage kernel exists for (dim, N)
+  bool pipe_ok = false;  // a pipelined DMMA stage kernel exists for (dim, N)
+  int kernel_mode = 0;   // 0 auto (pipelined DMMA, else DMMA, else generic), 1 generic, 2 pipelined DMMA, 3 warp-per-quad DMMA
   // device: mesh
   double *d_X0 = nullptr, *d_xv = nullptr, *d_vv = nullptr;
   int32_t *d_EToV = nullptr, *d_vmapP = nullptr;
@@ -145,7 +146,9 @@ int timed_stage(alegb_ctx* ctx, const StageArgs& a, cudaStream_t s) {
     }
     CU(cudaEventRecord(ctx->prof_events[ctx->prof_used], s));
   }
-  if (ctx->mma_ok && ctx->kernel_mode != 1) CU(launch_stage_mma(ctx->ref.dim, ctx->ref.N, a, ctx->num_sms, s));
+  const int mode = ctx->kernel_mode;
+  if (ctx->pipe_ok && (mode == 0 || mode == 2)) CU(launch_stage_pipe(ctx->ref.dim, ctx->ref.N, a, ctx->num_sms, s));
+  else if (ctx->mma_ok && (mode == 0 || mode == 3)) CU(launch_stage_mma(ctx->ref.dim, ctx->ref.N, a, ctx->num_sms, s));
   else CU(launch_stage(ctx->ref.dim, ctx->ref.N, a, ctx->num_sms, s));
   ctx->launches++;
   if (rec) {
@@ -267,6 +270,7 @@ int alegb_create(alegb_ctx** out, int dim, int N, int cuda_device) {
   // operators in DMMA fragment order: lane l of fragment (row tile nb, k-step ks) holds A[8 nb + l/4][4 ks + l%4]
   MmaLayout L{};
   ctx->mma_ok = mma_layout(dim, N, L) && configure_stage_mma(dim, N) == cudaSuccess;
+  ctx->pipe_ok = ctx->mma_ok && configure_stage_pipe(dim, N) == cudaSuccess;
   if (ctx->mma_ok) {
     std::vector<double> Av((size_t)dim * L.NB * L.KS * 32, 0.0), Al((size_t)r.Nfaces * L.NB * L.KF * 32, 0.0);
     for (int a = 0; a < dim; ++a)
@@ -622,8 +626,9 @@ int alegb_sark_coefficients(double gamma, double* a, double* b) {
 
 int alegb_set_kernel(alegb_ctx* ctx, int kind) {
   if (!ctx) return ALEGB_INVALID_ARG;
-  if (kind < 0 || kind > 2) return fail(ctx, ALEGB_INVALID_ARG, "kernel kind must be 0 (auto), 1 (generic) or 2 (DMMA)");
-  if (kind == 2 && !ctx->mma_ok) return fail(ctx, ALEGB_UNSUPPORTED, "no DMMA stage kernel for this (dim, N)");
+  if (kind < 0 || kind > 3) return fail(ctx, ALEGB_INVALID_ARG, "kernel kind must be 0 (auto), 1 (generic), 2 (pipelined DMMA) or 3 (warp-per-quad DMMA)");
+  if (kind == 2 && !ctx->pipe_ok) return fail(ctx, ALEGB_UNSUPPORTED, "no pipelined DMMA stage kernel for this (dim, N)");
+  if (kind == 3 && !ctx->mma_ok) return fail(ctx, ALEGB_UNSUPPORTED, "no DMMA stage kernel for this (dim, N)");
   ctx->kernel_mode = kind;
   return ALEGB_OK;
 }

@@ -94,4 +94,8 @@ bool mma_layout(int dim, int N, MmaLayout& L);       // false if (dim, N) has no
 cudaError_t configure_stage_mma(int dim, int N);
 cudaError_t launch_stage_mma(int dim, int N, const StageArgs& a, int num_sms, cudaStream_t s);
 
+// pipelined tensor-core stage kernel (producer / consumer warps), stage_pipe.cu; same operator fragments
+cudaError_t configure_stage_pipe(int dim, int N);     // cudaErrorInvalidValue if (dim, N) has no such kernel
+cudaError_t launch_stage_pipe(int dim, int N, const StageArgs& a, int num_sms, cudaStream_t s);
+
 }  // namespace alegb

@@ -1,0 +1,493 @@
+// Fused stage kernel, pipelined tensor-core version (DMMA, mma.sync.m8n8k4.f64) for sm_100a.
+//
+// Why this shape (profiles/r1_v2_mma_stage_kernel.md): on the 3-D configurations the stage is bound by the fp64
+// datapath (380 flop per degree of freedom against 38 B), and the warp-per-4-elements DMMA kernel kept that datapath
+// only ~50 % busy because each of its 8 warps serialised  tile load -> contraction -> neighbour gathers -> contraction
+// -> update loads  with every global-memory latency exposed.  Here a persistent CTA is split into
+//
+//   producer warps  stream "quads" (4 consecutive elements) into a ring of shared-memory slots: the q tile
+//                   (cp.async, padded rows), per-element metric data, per-face data, and the complete upwind flux
+//                   tile of the quad (a5: trace gather through vmapP, boundary states, eq. 7) -- all global-memory
+//                   latency of a3-a5 lives here, overlapped with the contractions of earlier quads;
+//   consumer warps  take work items (quad, block of 8 nodes): D_r,D_s,D_t contraction on the tensor cores (a3),
+//                   point-wise volume terms on the accumulator registers (a3, a4), LIFT contraction into the same
+//                   registers (a5), SARK update and stores (a6).
+//
+// Slots are handed over with mbarriers (full: producers -> consumers, empty: consumers -> producers).
+// DMMA operand layout as in stage_mma.cu: rows = nodes (blocks of 8), columns = (element 0..3) x (field pair
+// member), so lane (g = lane/4, c = lane%4) of a consumer holds every field of node 8*nb+g of element c.
+#include "alegb_internal.h"
+#include "device_common.cuh"
+
+namespace alegb {
+
+namespace pipe {
+
+__host__ __device__ constexpr int stride_pad(int x) {
+  // smallest s >= x with s = 4 (mod 16): B-fragment loads (8 rows x 4 consecutive doubles) are then conflict-free
+  int s = x;
+  while (s % 16 != 4) ++s;
+  return s;
+}
+
+template <int DIM, int N>
+struct Cfg {
+  static constexpr int Np = DIM == 2 ? (N + 1) * (N + 2) / 2 : (N + 1) * (N + 2) * (N + 3) / 6;
+  static constexpr int Nfp = DIM == 2 ? N + 1 : (N + 1) * (N + 2) / 2;
+  static constexpr int Nfaces = DIM + 1;
+  static constexpr int NFN = Nfaces * Nfp;
+  static constexpr int Nf = DIM == 2 ? 6 : 10;
+  static constexpr int NT = Nf / 2;            // column tiles (field pairs)
+  static constexpr int NB = (Np + 7) / 8;      // node blocks (row tiles) = work items per quad
+  static constexpr int KS = (Np + 3) / 4;      // k-steps of the volume contraction
+  static constexpr int KF = (Nfp + 3) / 4;     // k-steps of the surface contraction, per face
+  static constexpr int S = stride_pad(4 * KS);             // node stride of a q-tile row
+  static constexpr int SG = stride_pad(4 * KF * Nfaces);   // face-node stride of a flux-tile row
+  static constexpr int EG = 4;                 // elements per quad
+  static constexpr int PW = 4;                 // producer warps
+  static constexpr int CW = 8;                 // consumer warps (12 warps = 3 per SM sub-partition -> 168 registers)
+  static constexpr int NS = 4;                 // slots in the ring
+  static constexpr int Threads = (PW + CW) * 32;
+  static constexpr int PT = PW * 32;           // producer threads
+  static constexpr int NTASK = EG * NFN;       // flux tasks per quad
+  static constexpr int ROUNDS = (NTASK + PT - 1) / PT;
+  // slot layout, in doubles
+  static constexpr int off_gt = EG * Nf * S;
+  static constexpr int off_eg = off_gt + EG * Nf * SG;       // per element: G[DIM*DIM], W[(DIM+1)*DIM]
+  static constexpr int EGS = 24;
+  static constexpr int off_fg = off_eg + EG * EGS;           // per (element, face): nh[DIM], Fscale, VN[DIM+1]
+  static constexpr int FGS = 8;
+  static constexpr int off_int = off_fg + EG * Nfaces * FGS; // ints: pml[EG], tag[EG*Nfaces]
+  static constexpr int slot_doubles = off_int + (EG + EG * Nfaces + 1) / 2 + 1;
+  static constexpr int avol_doubles = DIM * NB * KS * 32;
+  static constexpr int alift_doubles = Nfaces * NB * KF * 32;
+  static constexpr int lam_doubles = NB * 8 * (DIM + 1);
+  static constexpr size_t smem_bytes = (size_t)(avol_doubles + alift_doubles + lam_doubles + NS * slot_doubles) * 8 +
+                                       (size_t)NFN * 4 + 2 * NS * 8 + 16;
+  static constexpr bool supported = smem_bytes <= 227 * 1024;
+};
+
+__device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+               : "+d"(c0), "+d"(c1)
+               : "d"(a), "d"(b));
+}
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void cp_async8(double* dst, const double* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void prefetch_l2(const void* p, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void producer_sync(int nthreads) {
+  asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
+}
+
+}  // namespace pipe
+
+template <int DIM, int N>
+__global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kernel(StageArgs a) {
+  using namespace pipe;
+  using C = Cfg<DIM, N>;
+  constexpr int Np = C::Np, Nfp = C::Nfp, Nfaces = C::Nfaces, NFN = C::NFN, Nf = C::Nf, NT = C::NT, NB = C::NB;
+  constexpr int KS = C::KS, KF = C::KF, S = C::S, SG = C::SG, EG = C::EG, NS = C::NS, PT = C::PT;
+  extern __shared__ double smem[];
+  double* sAvol = smem;                              // [DIM][NB][KS][32] fragment order
+  double* sAlift = sAvol + C::avol_doubles;          // [Nfaces][NB][KF][32]
+  double* slam = sAlift + C::alift_doubles;          // [NB*8][DIM+1], rows >= Np repeat the last node
+  double* sslots = slam + C::lam_doubles;            // [NS][slot_doubles]
+  uint64_t* full = reinterpret_cast<uint64_t*>(sslots + NS * C::slot_doubles);
+  uint64_t* empty = full + NS;
+  int* sfmask = reinterpret_cast<int*>(empty + NS);
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+  for (int x = tid; x < C::avol_doubles; x += C::Threads) sAvol[x] = a.Avol[x];
+  for (int x = tid; x < C::alift_doubles; x += C::Threads) sAlift[x] = a.Alift[x];
+  for (int x = tid; x < NB * 8; x += C::Threads) {
+    const int n = x < Np ? x : Np - 1;
+#pragma unroll
+    for (int v = 0; v <= DIM; ++v) slam[x * (DIM + 1) + v] = a.lam[n * (DIM + 1) + v];
+  }
+  for (int x = tid; x < NFN; x += C::Threads) sfmask[x] = a.fmask[x];
+  // zero the slots once: the k-padding of both tiles (j >= Np, m >= Nfp) is never written again and multiplies as 0
+  for (int x = tid; x < NS * C::slot_doubles; x += C::Threads) sslots[x] = 0.0;
+  if (tid == 0) {
+    for (int s = 0; s < NS; ++s) {
+      mbar_init(&full[s], PT);
+      mbar_init(&empty[s], NB * 32);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  const double cs = a.c;
+  const int64_t nquads = (a.K + EG - 1) / EG;
+  const int nq_cta = (int)((nquads - blockIdx.x + gridDim.x - 1) / gridDim.x);   // quads blockIdx.x + ql*gridDim.x
+
+  if (warp < C::PW) {
+    // =================================================================================================== producers
+    const int pt = tid;
+    constexpr int ROUNDS = C::ROUNDS;
+    int task_fe[ROUNDS], task_m[ROUNDS];
+#pragma unroll
+    for (int r = 0; r < ROUNDS; ++r) {
+      const int task = r * PT + pt;
+      task_fe[r] = task / NFN;
+      task_m[r] = task - task_fe[r] * NFN;
+    }
+    int idx_next[ROUNDS];
+    {
+      const int64_t e0 = (int64_t)blockIdx.x * EG;
+#pragma unroll
+      for (int r = 0; r < ROUNDS; ++r) {
+        const int64_t ee = e0 + task_fe[r];
+        idx_next[r] = (nq_cta > 0 && r * PT + pt < C::NTASK && ee < a.K) ? __ldg(a.vmapP + ee * NFN + task_m[r]) : -1;
+      }
+    }
+    for (int ql = 0; ql < nq_cta; ++ql) {
+      const int64_t quad = (int64_t)ql * gridDim.x + blockIdx.x;
+      const int64_t e0 = quad * EG;
+      const int nel = (a.K - e0) < EG ? (int)(a.K - e0) : EG;
+      const int slot = ql % NS, use = ql / NS;
+      double* qt = sslots + slot * C::slot_doubles;
+      double* gt = qt + C::off_gt;
+      double* eg = qt + C::off_eg;
+      double* fg = qt + C::off_fg;
+      int* si = reinterpret_cast<int*>(qt + C::off_int);
+      if (use > 0) mbar_wait(&empty[slot], (use - 1) & 1);
+      // ---- q tile of the quad, rows (element, field), node stride S
+      {
+        const double* src = a.q_in + e0 * Nf * Np;
+        const int total = nel * Nf * Np;
+        for (int x = pt; x < total; x += PT) {
+          const int row = x / Np, j = x - row * Np;
+          cp_async8(qt + row * S + j, src + x);
+        }
+      }
+      // ---- L2 prefetch of the a6 inputs the consumers will read for this quad
+      if (pt == 0) {
+        const uint32_t bytes = (uint32_t)(nel * Nf * Np * 8);
+        const int64_t off = e0 * Nf * Np;
+        if (a.q_n != nullptr && a.q_n != a.q_in && (a.q_out || a.acc_out)) prefetch_l2(a.q_n + off, bytes);
+        if (a.F0_in != nullptr) prefetch_l2(a.F0_in + off, bytes);
+        if (a.acc_in != nullptr) prefetch_l2(a.acc_in + off, bytes);
+      }
+      // ---- exterior traces q+ of my face nodes (indices were fetched one quad ahead), then next quad's indices
+      double qP[ROUNDS][Nf];
+#pragma unroll
+      for (int r = 0; r < ROUNDS; ++r) {
+        const int idP = idx_next[r];
+        if (idP >= 0) {
+          const int eP = idP / Np, nP = idP - eP * Np;
+          const double* qp = a.q_in + (int64_t)eP * Nf * Np + nP;
+#pragma unroll
+          for (int k = 0; k < Nf; ++k) qP[r][k] = __ldg(qp + k * Np);
+        } else {
+#pragma unroll
+          for (int k = 0; k < Nf; ++k) qP[r][k] = 0.0;
+        }
+      }
+      bool valid[ROUNDS];
+#pragma unroll
+      for (int r = 0; r < ROUNDS; ++r) valid[r] = idx_next[r] >= 0;
+      if (ql + 1 < nq_cta) {
+        const int64_t e1 = (quad + gridDim.x) * EG;
+#pragma unroll
+        for (int r = 0; r < ROUNDS; ++r) {
+          const int64_t ee = e1 + task_fe[r];
+          idx_next[r] = (r * PT + pt < C::NTASK && ee < a.K) ? __ldg(a.vmapP + ee * NFN + task_m[r]) : -1;
+        }
+      }
+      // ---- per-element data: metrics G[a][d] and W[v][a] = sum_d vvel[v][d] G[a][d]  (v_G . grad = sum_a w_a D_a)
+      if (pt < EG) {
+        const int el = pt;
+        double G[DIM * DIM], W[(DIM + 1) * DIM];
+        int pml = -1;
+        if (el < nel) {
+          const int64_t e = e0 + el;
+          const double* vg = a.vgeo + e * (DIM * DIM + 1);
+          const double* ve = a.vvel + e * (DIM + 1) * DIM;
+#pragma unroll
+          for (int x = 0; x < DIM * DIM; ++x) G[x] = vg[x];
+#pragma unroll
+          for (int v = 0; v <= DIM; ++v)
+#pragma unroll
+            for (int r = 0; r < DIM; ++r) {
+              double s = 0.0;
+#pragma unroll
+              for (int d = 0; d < DIM; ++d) s = fma(ve[v * DIM + d], G[r * DIM + d], s);
+              W[v * DIM + r] = s;
+            }
+          if (a.pml_index != nullptr && a.aux != nullptr) pml = a.pml_index[e];
+        } else {
+#pragma unroll
+          for (int x = 0; x < DIM * DIM; ++x) G[x] = 0.0;
+#pragma unroll
+          for (int x = 0; x < (DIM + 1) * DIM; ++x) W[x] = 0.0;
+        }
+#pragma unroll
+        for (int x = 0; x < DIM * DIM; ++x) eg[el * C::EGS + x] = G[x];
+#pragma unroll
+        for (int x = 0; x < (DIM + 1) * DIM; ++x) eg[el * C::EGS + DIM * DIM + x] = W[x];
+        si[el] = pml;
+      }
+      // ---- per-face data: unit normal, Fscale, VN[v] = vvel[v] . n  (v_n at a node = sum_v lambda_v VN[v], L196)
+      if (pt >= 32 && pt < 32 + EG * Nfaces) {
+        const int ef = pt - 32, el = ef / Nfaces, f = ef - el * Nfaces;
+        double out[C::FGS];
+#pragma unroll
+        for (int x = 0; x < C::FGS; ++x) out[x] = 0.0;
+        int tag = 0;
+        if (el < nel) {
+          const int64_t e = e0 + el;
+          const double* sg = a.sgeo + (e * Nfaces + f) * (DIM + 2);
+          const double* ve = a.vvel + e * (DIM + 1) * DIM;
+#pragma unroll
+          for (int d = 0; d < DIM; ++d) out[d] = sg[d];
+          out[DIM] = sg[DIM + 1];
+#pragma unroll
+          for (int v = 0; v <= DIM; ++v) {
+            double s = 0.0;
+#pragma unroll
+            for (int d = 0; d < DIM; ++d) s = fma(ve[v * DIM + d], out[d], s);
+            out[DIM + 1 + v] = s;
+          }
+          if (a.EToB) tag = a.EToB[e * Nfaces + f];
+        }
+#pragma unroll
+        for (int x = 0; x < C::FGS; ++x) fg[ef * C::FGS + x] = out[x];
+        si[EG + ef] = tag;
+      }
+      cp_async_wait_all();
+      producer_sync(PT);
+      // ---- a5: upwind flux at my face nodes (eq. 7; reading R7) into the flux tile
+#pragma unroll
+      for (int r = 0; r < ROUNDS; ++r) {
+        if (!valid[r]) continue;
+        const int fe = task_fe[r], m = task_m[r];
+        const int f = m / Nfp, mm = m - f * Nfp;
+        const int n = sfmask[m];
+        double qM[Nf];
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) qM[k] = qt[(fe * Nf + k) * S + n];
+        const double* fd = fg + (fe * Nfaces + f) * C::FGS;
+        double nh[DIM];
+#pragma unroll
+        for (int d = 0; d < DIM; ++d) nh[d] = fd[d];
+        const double Fscale = fd[DIM];
+        double vn = 0.0;
+#pragma unroll
+        for (int v = 0; v <= DIM; ++v) vn = fma(slam[n * (DIM + 1) + v], fd[DIM + 1 + v], vn);
+        const int tag = si[EG + fe * Nfaces + f];
+        if (tag == 1) {          // wall moving with the mesh (reading R11)
+          double vG[DIM];
+          node_velocity<DIM>(slam + n * (DIM + 1), a.vvel + (e0 + fe) * (DIM + 1) * DIM, vG);
+#pragma unroll
+          for (int k = 0; k < Nf; ++k) qP[r][k] = qM[k];
+#pragma unroll
+          for (int d = 0; d < DIM; ++d) qP[r][1 + d] = 2.0 * qM[0] * vG[d] / cs - qM[1 + d];
+        } else if (tag != 0) {   // far field
+#pragma unroll
+          for (int k = 0; k < Nf; ++k) qP[r][k] = a.q_inf[k];
+        }
+        double fl[Nf];
+        upwind_flux<DIM>(qM, qP[r], nh, cs, vn, Fscale, fl);
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) gt[(fe * Nf + k) * SG + f * 4 * KF + mm] = fl[k];
+      }
+      mbar_arrive(&full[slot]);
+    }
+  } else {
+    // =================================================================================================== consumers
+    const int cw = warp - C::PW;
+    const int g = lane >> 2, c = lane & 3;
+    // B-fragment column of this lane: column g  <->  element g/2, field 2t + (g&1); k index = c
+    const int bcol = (g >> 1) * Nf + (g & 1);
+    const bool qn_in_tile = a.q_n == a.q_in;
+    const bool want_update = a.q_out != nullptr || a.acc_out != nullptr;
+    const int nitems = nq_cta * NB;
+    for (int it = cw; it < nitems; it += C::CW) {
+      const int ql = it / NB, nb = it - ql * NB;
+      const int64_t quad = (int64_t)ql * gridDim.x + blockIdx.x;
+      const int64_t e0 = quad * EG;
+      const int nel = (a.K - e0) < EG ? (int)(a.K - e0) : EG;
+      const int slot = ql % NS, use = ql / NS;
+      const double* qt = sslots + slot * C::slot_doubles;
+      const double* gt = qt + C::off_gt;
+      const double* eg = qt + C::off_eg + c * C::EGS;
+      const int* si = reinterpret_cast<const int*>(qt + C::off_int);
+      mbar_wait(&full[slot], use & 1);
+
+      // ---- a3: reference derivatives D_a q of all fields at nodes 8nb..8nb+7 of the 4 elements (L103, L195)
+      double acc[DIM][NT][2];
+#pragma unroll
+      for (int d = 0; d < DIM; ++d)
+#pragma unroll
+        for (int t = 0; t < NT; ++t) acc[d][t][0] = acc[d][t][1] = 0.0;
+#pragma unroll
+      for (int ks = 0; ks < KS; ++ks) {
+        double bf[NT], af[DIM];
+#pragma unroll
+        for (int t = 0; t < NT; ++t) bf[t] = qt[(bcol + 2 * t) * S + 4 * ks + c];
+#pragma unroll
+        for (int d = 0; d < DIM; ++d) af[d] = sAvol[((d * NB + nb) * KS + ks) * 32 + lane];
+#pragma unroll
+        for (int d = 0; d < DIM; ++d)
+#pragma unroll
+          for (int t = 0; t < NT; ++t) dmma(acc[d][t][0], acc[d][t][1], af[d], bf[t]);
+      }
+      // ---- point-wise volume terms at node n of element c (eq. 9 first term, L107; a4 relaxation L115)
+      const int n = 8 * nb + g;
+      const int nn = n < Np ? n : Np - 1;
+      double V[NT][2];
+      {
+        double G[DIM * DIM], w[DIM];
+#pragma unroll
+        for (int x = 0; x < DIM * DIM; ++x) G[x] = eg[x];
+#pragma unroll
+        for (int r = 0; r < DIM; ++r) {
+          double s = 0.0;
+#pragma unroll
+          for (int v = 0; v <= DIM; ++v) s = fma(slam[n * (DIM + 1) + v], eg[DIM * DIM + v * DIM + r], s);
+          w[r] = s;   // w_r = v_G . grad(xi_r)
+        }
+        double st[Nf], qn[Nf], nt[Nf];
+        hermite_apply<DIM>(
+            [&](int d, int j) {
+              double s = 0.0;
+#pragma unroll
+              for (int r = 0; r < DIM; ++r) s = fma(G[r * DIM + d], acc[r][j >> 1][j & 1], s);
+              return s;   // d q_j / d x_d
+            },
+            st);
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) qn[k] = qt[(c * Nf + k) * S + nn];
+        relaxation<DIM>(qn, a.invtau, nt);
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) {
+          double v = fma(-cs, st[k], nt[k]);
+#pragma unroll
+          for (int r = 0; r < DIM; ++r) v = fma(w[r], acc[r][k >> 1][k & 1], v);
+          V[k >> 1][k & 1] = v;
+        }
+      }
+      const bool evalid = c < nel && n < Np;
+      const int64_t e = e0 + (c < nel ? c : 0);
+      const int64_t base = e * Nf * Np + nn;
+      const int pml = si[c];
+      if (pml >= 0) {   // absorbing layer (reading R12): - sum_d sigma_d q~^d
+#pragma unroll
+        for (int d = 0; d < DIM; ++d) {
+          const double sig = a.pml_sigma[(int64_t)pml * DIM + d];
+#pragma unroll
+          for (int k = 0; k < Nf; ++k)
+            V[k >> 1][k & 1] -= sig * a.aux[(((int64_t)pml * DIM + d) * Nf + k) * Np + nn];
+        }
+      }
+      // ---- a6 inputs, requested before the LIFT contraction so that their latency hides behind it
+      double uq[Nf], uf[Nf], ua[Nf];
+#pragma unroll
+      for (int k = 0; k < Nf; ++k) {
+        uq[k] = 0.0; uf[k] = 0.0; ua[k] = 0.0;
+        if (evalid && want_update) {
+          if (a.q_n != nullptr) uq[k] = qn_in_tile ? qt[(c * Nf + k) * S + nn] : __ldg(a.q_n + base + k * Np);
+          if (a.F0_in != nullptr) uf[k] = __ldg(a.F0_in + base + k * Np);
+          if (a.acc_in != nullptr) ua[k] = __ldg(a.acc_in + base + k * Np);
+        }
+      }
+      // ---- a5: LIFT contraction of the quad's flux tile into the same registers (L103, L196)
+#pragma unroll
+      for (int ks = 0; ks < Nfaces * KF; ++ks) {
+        double bf[NT];
+#pragma unroll
+        for (int t = 0; t < NT; ++t) bf[t] = gt[(bcol + 2 * t) * SG + 4 * ks + c];
+        const double af = sAlift[(((ks / KF) * NB + nb) * KF + (ks % KF)) * 32 + lane];
+#pragma unroll
+        for (int t = 0; t < NT; ++t) dmma(V[t][0], V[t][1], af, bf[t]);
+      }
+      // all reads of the slot are done
+      mbar_arrive(&empty[slot]);
+      // ---- a6: SARK stage update (L132-134), straight from the accumulator registers
+      if (evalid) {
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) {
+          const int64_t idx = base + k * Np;
+          const double F = V[k >> 1][k & 1];
+          if (a.F_out) a.F_out[idx] = F;
+          if (a.q_out) {
+            double v = a.coef.cq_n[k] * uq[k];
+            v = fma(a.coef.cq_f0[k], uf[k], v);
+            v = fma(a.coef.cq_acc, ua[k], v);
+            a.q_out[idx] = fma(a.coef.cq_f[k], F, v);
+          }
+          if (a.acc_out) {
+            double v = a.coef.ca_n[k] * uq[k];
+            v = fma(a.coef.ca_f0[k], uf[k], v);
+            v = fma(a.coef.ca_acc, ua[k], v);
+            a.acc_out[idx] = fma(a.coef.ca_f[k], F, v);
+          }
+        }
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+template <int DIM, int N>
+static cudaError_t launch_pipe_one(const StageArgs& a, int num_sms, cudaStream_t s, bool configure_only) {
+  using C = pipe::Cfg<DIM, N>;
+  if constexpr (!C::supported) {
+    return cudaErrorInvalidValue;
+  } else {
+    if (configure_only)
+      return cudaFuncSetAttribute(stage_pipe_kernel<DIM, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
+    const int64_t nquads = (a.K + C::EG - 1) / C::EG;
+    if (nquads == 0) return cudaSuccess;
+    int64_t grid = nquads < num_sms ? nquads : num_sms;
+    stage_pipe_kernel<DIM, N><<<(int)grid, C::Threads, C::smem_bytes, s>>>(a);
+    return cudaGetLastError();
+  }
+}
+
+#define ALEGB_PIPE_DISPATCH(...)                                  \
+  switch (dim * 10 + N) {                                         \
+    case 21: return launch_pipe_one<2, 1>(__VA_ARGS__);           \
+    case 22: return launch_pipe_one<2, 2>(__VA_ARGS__);           \
+    case 23: return launch_pipe_one<2, 3>(__VA_ARGS__);           \
+    case 24: return launch_pipe_one<2, 4>(__VA_ARGS__);           \
+    case 25: return launch_pipe_one<2, 5>(__VA_ARGS__);           \
+    case 31: return launch_pipe_one<3, 1>(__VA_ARGS__);           \
+    case 32: return launch_pipe_one<3, 2>(__VA_ARGS__);           \
+    case 33: return launch_pipe_one<3, 3>(__VA_ARGS__);           \
+    case 34: return launch_pipe_one<3, 4>(__VA_ARGS__);           \
+    default: return cudaErrorInvalidValue;                        \
+  }
+
+cudaError_t launch_stage_pipe(int dim, int N, const StageArgs& a, int num_sms, cudaStream_t s) {
+  ALEGB_PIPE_DISPATCH(a, num_sms, s, false)
+}
+cudaError_t configure_stage_pipe(int dim, int N) {
+  StageArgs a{};
+  ALEGB_PIPE_DISPATCH(a, 0, nullptr, true)
+}
+
+}  // namespace alegb

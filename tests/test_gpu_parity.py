@@ -78,7 +78,7 @@ def make_case(name, refs):
 
 
 CASES = ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "tri_N1", "tri_N5", "tet_N2", "tet_N5"]
-KERNELS = [1, 2]        # alegb_set_kernel: 1 = generic DFMA stage kernel, 2 = tensor-core DMMA stage kernel
+KERNELS = [1, 2, 3]     # alegb_set_kernel: 1 = generic DFMA kernel, 2 = pipelined DMMA kernel, 3 = warp-per-quad DMMA kernel
 
 
 def make_ctx(B, cfg, kernel):
@@ -86,7 +86,7 @@ def make_ctx(B, cfg, kernel):
     try:
         ctx.alegb_set_kernel(kernel)
     except B.AlegbError as e:
-        assert e.status == B.UNSUPPORTED and kernel == 2
+        assert e.status == B.UNSUPPORTED and kernel in (2, 3)
         ctx.close()
         pytest.skip("no DMMA kernel for dim=%d N=%d (the generic kernel covers it)" % (cfg["dim"], cfg["N"]))
     return ctx
