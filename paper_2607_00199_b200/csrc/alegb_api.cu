@@ -22,7 +22,7 @@ struct alegb_ctx {
   MotionArgs motion{};
   std::vector<int32_t> vmapM_host, vmapP_host, pml_elems_host;
   // device: operators
-  double *d_Dt = nullptr, *d_LIFTt = nullptr, *d_lam = nullptr, *d_Avol = nullptr, *d_Alift = nullptr;
+  double *d_Dt = nullptr, *d_LIFTt = nullptr, *d_lam = nullptr, *d_Avol = nullptr, *d_Alift = nullptr, *d_AliftP = nullptr;
   int32_t* d_fmask = nullptr;
   bool mma_ok = false;   // a warp-per-quad DMMA stage kernel exists for (dim, N)
   bool pipe_ok = false;  // a pipelined DMMA stage kernel exists for (dim, N)
@@ -111,7 +111,7 @@ void fill_common(const alegb_ctx* ctx, StageArgs& a) {
   a.vmapP = ctx->d_vmapP; a.EToB = ctx->d_EToB;
   a.pml_index = ctx->d_pml_index; a.pml_sigma = ctx->d_pml_sigma;
   a.Dt_ops = ctx->d_Dt; a.LIFTt = ctx->d_LIFTt; a.lam = ctx->d_lam; a.fmask = ctx->d_fmask;
-  a.Avol = ctx->d_Avol; a.Alift = ctx->d_Alift;
+  a.Avol = ctx->d_Avol; a.Alift = ctx->d_Alift; a.AliftP = ctx->d_AliftP;
   a.c = ctx->c; a.invtau = ctx->invtau;
   for (int k = 0; k < kMaxFields; ++k) a.q_inf[k] = ctx->q_inf[k];
 }
@@ -287,8 +287,17 @@ int alegb_create(alegb_ctx** out, int dim, int N, int cuda_device) {
             const int row = 8 * nb + l / 4, m = 4 * ks + l % 4;
             if (row < Np && m < r.Nfp) Al[(((size_t)f * L.NB + nb) * L.KF + ks) * 32 + l] = r.LIFT[row * ncol + f * r.Nfp + m];
           }
+    const int KFT = (ncol + 3) / 4;   // pipelined kernel: the faces' k ranges packed back to back, m = f*Nfp + mm
+    std::vector<double> Alp((size_t)L.NB * KFT * 32, 0.0);
+    for (int nb = 0; nb < L.NB; ++nb)
+      for (int ks = 0; ks < KFT; ++ks)
+        for (int l = 0; l < 32; ++l) {
+          const int row = 8 * nb + l / 4, m = 4 * ks + l % 4;
+          if (row < Np && m < ncol) Alp[((size_t)nb * KFT + ks) * 32 + l] = r.LIFT[row * ncol + m];
+        }
     if (upload(ctx, &ctx->d_Avol, Av.data(), Av.size()) != cudaSuccess ||
-        upload(ctx, &ctx->d_Alift, Al.data(), Al.size()) != cudaSuccess) {
+        upload(ctx, &ctx->d_Alift, Al.data(), Al.size()) != cudaSuccess ||
+        upload(ctx, &ctx->d_AliftP, Alp.data(), Alp.size()) != cudaSuccess) {
       alegb_destroy(ctx);
       return ALEGB_CUDA_ERROR;
     }
@@ -313,7 +322,7 @@ int alegb_destroy(alegb_ctx* ctx) {
   free_mesh(ctx);
   for (cudaEvent_t ev : ctx->prof_events) cudaEventDestroy(ev);
   dev_free(ctx->d_Dt); dev_free(ctx->d_LIFTt); dev_free(ctx->d_lam); dev_free(ctx->d_fmask);
-  dev_free(ctx->d_Avol); dev_free(ctx->d_Alift);
+  dev_free(ctx->d_Avol); dev_free(ctx->d_Alift); dev_free(ctx->d_AliftP);
   delete ctx;
   return ALEGB_OK;
 }

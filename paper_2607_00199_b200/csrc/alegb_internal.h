@@ -41,6 +41,7 @@ struct StageArgs {
   const int32_t* fmask;  // [Nfaces*Nfp]
   const double* Avol;    // DMMA path: D_a in fragment order [dim][NB][KS][32]
   const double* Alift;   // DMMA path: LIFT in fragment order [Nfaces][NB][KF][32]
+  const double* AliftP;  // DMMA path, faces packed along k: [NB][ceil(Nfaces*Nfp/4)][32]
   // physics
   double c, invtau;
   double q_inf[kMaxFields];

@@ -40,9 +40,9 @@ struct Cfg {
   static constexpr int NT = Nf / 2;            // column tiles (field pairs)
   static constexpr int NB = (Np + 7) / 8;      // node blocks (row tiles) = work items per quad
   static constexpr int KS = (Np + 3) / 4;      // k-steps of the volume contraction
-  static constexpr int KF = (Nfp + 3) / 4;     // k-steps of the surface contraction, per face
-  static constexpr int S = stride_pad(4 * KS);             // node stride of a q-tile row
-  static constexpr int SG = stride_pad(4 * KF * Nfaces);   // face-node stride of a flux-tile row
+  static constexpr int KFT = (NFN + 3) / 4;    // k-steps of the surface contraction (all faces packed: m = f*Nfp + mm)
+  static constexpr int S = stride_pad(4 * KS);     // node stride of a q-tile row
+  static constexpr int SG = stride_pad(4 * KFT);   // face-node stride of a flux-tile row
   static constexpr int EG = 4;                 // elements per quad
   static constexpr int PW = 4;                 // producer warps
   static constexpr int CW = 8;                 // consumer warps (12 warps = 3 per SM sub-partition -> 168 registers)
@@ -51,16 +51,19 @@ struct Cfg {
   static constexpr int PT = PW * 32;           // producer threads
   static constexpr int NTASK = EG * NFN;       // flux tasks per quad
   static constexpr int ROUNDS = (NTASK + PT - 1) / PT;
+  // per-element geometry records, copied raw from the geometry kernel's arrays
+  static constexpr int VG = DIM * DIM + 1;         // vgeo: d xi_a / d x_d, J
+  static constexpr int VV = (DIM + 1) * DIM;       // vvel: vertex velocities
+  static constexpr int SGE = Nfaces * (DIM + 2);   // sgeo: per face unit normal, sJ, Fscale
   // slot layout, in doubles
   static constexpr int off_gt = EG * Nf * S;
-  static constexpr int off_eg = off_gt + EG * Nf * SG;       // per element: G[DIM*DIM], W[(DIM+1)*DIM]
-  static constexpr int EGS = 24;
-  static constexpr int off_fg = off_eg + EG * EGS;           // per (element, face): nh[DIM], Fscale, VN[DIM+1]
-  static constexpr int FGS = 8;
-  static constexpr int off_int = off_fg + EG * Nfaces * FGS; // ints: pml[EG], tag[EG*Nfaces]
+  static constexpr int off_vg = off_gt + EG * Nf * SG;
+  static constexpr int off_vv = off_vg + EG * VG;
+  static constexpr int off_sg = off_vv + EG * VV;
+  static constexpr int off_int = off_sg + EG * SGE;          // ints: pml[EG], tag[EG*Nfaces]
   static constexpr int slot_doubles = off_int + (EG + EG * Nfaces + 1) / 2 + 1;
   static constexpr int avol_doubles = DIM * NB * KS * 32;
-  static constexpr int alift_doubles = Nfaces * NB * KF * 32;
+  static constexpr int alift_doubles = NB * KFT * 32;
   static constexpr int lam_doubles = NB * 8 * (DIM + 1);
   static constexpr size_t smem_bytes = (size_t)(avol_doubles + alift_doubles + lam_doubles + NS * slot_doubles) * 8 +
                                        (size_t)NFN * 4 + 2 * NS * 8 + 16;
@@ -94,7 +97,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 __device__ __forceinline__ void cp_async8(double* dst, const double* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
 }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int NPENDING>
+__device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(NPENDING) : "memory"); }
 __device__ __forceinline__ void prefetch_l2(const void* p, uint32_t bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
@@ -109,10 +114,10 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
   using namespace pipe;
   using C = Cfg<DIM, N>;
   constexpr int Np = C::Np, Nfp = C::Nfp, Nfaces = C::Nfaces, NFN = C::NFN, Nf = C::Nf, NT = C::NT, NB = C::NB;
-  constexpr int KS = C::KS, KF = C::KF, S = C::S, SG = C::SG, EG = C::EG, NS = C::NS, PT = C::PT;
+  constexpr int KS = C::KS, KFT = C::KFT, S = C::S, SG = C::SG, EG = C::EG, NS = C::NS, PT = C::PT;
   extern __shared__ double smem[];
   double* sAvol = smem;                              // [DIM][NB][KS][32] fragment order
-  double* sAlift = sAvol + C::avol_doubles;          // [Nfaces][NB][KF][32]
+  double* sAlift = sAvol + C::avol_doubles;          // [NB][KFT][32]
   double* slam = sAlift + C::alift_doubles;          // [NB*8][DIM+1], rows >= Np repeat the last node
   double* sslots = slam + C::lam_doubles;            // [NS][slot_doubles]
   uint64_t* full = reinterpret_cast<uint64_t*>(sslots + NS * C::slot_doubles);
@@ -121,14 +126,14 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
   for (int x = tid; x < C::avol_doubles; x += C::Threads) sAvol[x] = a.Avol[x];
-  for (int x = tid; x < C::alift_doubles; x += C::Threads) sAlift[x] = a.Alift[x];
+  for (int x = tid; x < C::alift_doubles; x += C::Threads) sAlift[x] = a.AliftP[x];
   for (int x = tid; x < NB * 8; x += C::Threads) {
     const int n = x < Np ? x : Np - 1;
 #pragma unroll
     for (int v = 0; v <= DIM; ++v) slam[x * (DIM + 1) + v] = a.lam[n * (DIM + 1) + v];
   }
   for (int x = tid; x < NFN; x += C::Threads) sfmask[x] = a.fmask[x];
-  // zero the slots once: the k-padding of both tiles (j >= Np, m >= Nfp) is never written again and multiplies as 0
+  // zero the slots once: the k-padding of both tiles (j >= Np, m >= NFN) is never written again and multiplies as 0
   for (int x = tid; x < NS * C::slot_doubles; x += C::Threads) sslots[x] = 0.0;
   if (tid == 0) {
     for (int s = 0; s < NS; ++s) {
@@ -145,6 +150,8 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
 
   if (warp < C::PW) {
     // =================================================================================================== producers
+    // Every global read of a quad is asynchronous (cp.async straight into its slot) and issued one quad ahead of
+    // the flux arithmetic, so the producers never sit on a load: iteration ql issues quad ql+1, then computes quad ql.
     const int pt = tid;
     constexpr int ROUNDS = C::ROUNDS;
     int task_fe[ROUNDS], task_m[ROUNDS];
@@ -154,27 +161,24 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       task_fe[r] = task / NFN;
       task_m[r] = task - task_fe[r] * NFN;
     }
-    int idx_next[ROUNDS];
-    {
-      const int64_t e0 = (int64_t)blockIdx.x * EG;
+    int idx_next[ROUNDS];   // vmapP entries of my face nodes in the quad that is issued next
+    int meta_next = 0;      // pml index (threads < EG) / boundary tag (threads 32 .. 32+EG*Nfaces) of that quad
+
+    auto load_indices = [&](int ql) {
+      const int64_t e0 = ((int64_t)ql * gridDim.x + blockIdx.x) * EG;
 #pragma unroll
       for (int r = 0; r < ROUNDS; ++r) {
         const int64_t ee = e0 + task_fe[r];
-        idx_next[r] = (nq_cta > 0 && r * PT + pt < C::NTASK && ee < a.K) ? __ldg(a.vmapP + ee * NFN + task_m[r]) : -1;
+        idx_next[r] = (ql < nq_cta && r * PT + pt < C::NTASK && ee < a.K) ? __ldg(a.vmapP + ee * NFN + task_m[r]) : -1;
       }
-    }
-    for (int ql = 0; ql < nq_cta; ++ql) {
-      const int64_t quad = (int64_t)ql * gridDim.x + blockIdx.x;
-      const int64_t e0 = quad * EG;
+    };
+    auto issue = [&](int ql) {
+      const int64_t e0 = ((int64_t)ql * gridDim.x + blockIdx.x) * EG;
       const int nel = (a.K - e0) < EG ? (int)(a.K - e0) : EG;
       const int slot = ql % NS, use = ql / NS;
       double* qt = sslots + slot * C::slot_doubles;
-      double* gt = qt + C::off_gt;
-      double* eg = qt + C::off_eg;
-      double* fg = qt + C::off_fg;
-      int* si = reinterpret_cast<int*>(qt + C::off_int);
       if (use > 0) mbar_wait(&empty[slot], (use - 1) & 1);
-      // ---- q tile of the quad, rows (element, field), node stride S
+      // q tile of the quad, rows (element, field), node stride S
       {
         const double* src = a.q_in + e0 * Nf * Np;
         const int total = nel * Nf * Np;
@@ -183,136 +187,96 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
           cp_async8(qt + row * S + j, src + x);
         }
       }
-      // ---- L2 prefetch of the a6 inputs the consumers will read for this quad
-      if (pt == 0) {
-        const uint32_t bytes = (uint32_t)(nel * Nf * Np * 8);
-        const int64_t off = e0 * Nf * Np;
-        if (a.q_n != nullptr && a.q_n != a.q_in && (a.q_out || a.acc_out)) prefetch_l2(a.q_n + off, bytes);
-        if (a.F0_in != nullptr) prefetch_l2(a.F0_in + off, bytes);
-        if (a.acc_in != nullptr) prefetch_l2(a.acc_in + off, bytes);
-      }
-      // ---- exterior traces q+ of my face nodes (indices were fetched one quad ahead), then next quad's indices
-      double qP[ROUNDS][Nf];
+      // exterior traces q+ of my face nodes, into the flux tile (the flux overwrites them in place)
 #pragma unroll
       for (int r = 0; r < ROUNDS; ++r) {
         const int idP = idx_next[r];
         if (idP >= 0) {
           const int eP = idP / Np, nP = idP - eP * Np;
           const double* qp = a.q_in + (int64_t)eP * Nf * Np + nP;
+          double* dst = qt + C::off_gt + task_fe[r] * Nf * SG + task_m[r];
 #pragma unroll
-          for (int k = 0; k < Nf; ++k) qP[r][k] = __ldg(qp + k * Np);
-        } else {
-#pragma unroll
-          for (int k = 0; k < Nf; ++k) qP[r][k] = 0.0;
+          for (int k = 0; k < Nf; ++k) cp_async8(dst + k * SG, qp + k * Np);
         }
       }
-      bool valid[ROUNDS];
-#pragma unroll
-      for (int r = 0; r < ROUNDS; ++r) valid[r] = idx_next[r] >= 0;
-      if (ql + 1 < nq_cta) {
-        const int64_t e1 = (quad + gridDim.x) * EG;
-#pragma unroll
-        for (int r = 0; r < ROUNDS; ++r) {
-          const int64_t ee = e1 + task_fe[r];
-          idx_next[r] = (r * PT + pt < C::NTASK && ee < a.K) ? __ldg(a.vmapP + ee * NFN + task_m[r]) : -1;
-        }
-      }
-      // ---- per-element data: metrics G[a][d] and W[v][a] = sum_d vvel[v][d] G[a][d]  (v_G . grad = sum_a w_a D_a)
+      // geometric factors of the quad's elements, raw (a2's output; contiguous per quad)
+      for (int x = pt; x < nel * C::VG; x += PT) cp_async8(qt + C::off_vg + x, a.vgeo + e0 * C::VG + x);
+      for (int x = pt; x < nel * C::VV; x += PT) cp_async8(qt + C::off_vv + x, a.vvel + e0 * C::VV + x);
+      for (int x = pt; x < nel * C::SGE; x += PT) cp_async8(qt + C::off_sg + x, a.sgeo + e0 * C::SGE + x);
+      // integer records, through a register (stored one iteration later)
+      meta_next = pt < EG ? -1 : 0;
       if (pt < EG) {
-        const int el = pt;
-        double G[DIM * DIM], W[(DIM + 1) * DIM];
-        int pml = -1;
-        if (el < nel) {
-          const int64_t e = e0 + el;
-          const double* vg = a.vgeo + e * (DIM * DIM + 1);
-          const double* ve = a.vvel + e * (DIM + 1) * DIM;
-#pragma unroll
-          for (int x = 0; x < DIM * DIM; ++x) G[x] = vg[x];
-#pragma unroll
-          for (int v = 0; v <= DIM; ++v)
-#pragma unroll
-            for (int r = 0; r < DIM; ++r) {
-              double s = 0.0;
-#pragma unroll
-              for (int d = 0; d < DIM; ++d) s = fma(ve[v * DIM + d], G[r * DIM + d], s);
-              W[v * DIM + r] = s;
-            }
-          if (a.pml_index != nullptr && a.aux != nullptr) pml = a.pml_index[e];
-        } else {
-#pragma unroll
-          for (int x = 0; x < DIM * DIM; ++x) G[x] = 0.0;
-#pragma unroll
-          for (int x = 0; x < (DIM + 1) * DIM; ++x) W[x] = 0.0;
-        }
-#pragma unroll
-        for (int x = 0; x < DIM * DIM; ++x) eg[el * C::EGS + x] = G[x];
-#pragma unroll
-        for (int x = 0; x < (DIM + 1) * DIM; ++x) eg[el * C::EGS + DIM * DIM + x] = W[x];
-        si[el] = pml;
+        if (pt < nel && a.pml_index != nullptr && a.aux != nullptr) meta_next = __ldg(a.pml_index + e0 + pt);
+      } else if (pt >= 32 && pt < 32 + EG * Nfaces) {
+        const int ef = pt - 32;
+        if (ef < nel * Nfaces && a.EToB != nullptr) meta_next = a.EToB[e0 * Nfaces + ef];
       }
-      // ---- per-face data: unit normal, Fscale, VN[v] = vvel[v] . n  (v_n at a node = sum_v lambda_v VN[v], L196)
-      if (pt >= 32 && pt < 32 + EG * Nfaces) {
-        const int ef = pt - 32, el = ef / Nfaces, f = ef - el * Nfaces;
-        double out[C::FGS];
-#pragma unroll
-        for (int x = 0; x < C::FGS; ++x) out[x] = 0.0;
-        int tag = 0;
-        if (el < nel) {
-          const int64_t e = e0 + el;
-          const double* sg = a.sgeo + (e * Nfaces + f) * (DIM + 2);
-          const double* ve = a.vvel + e * (DIM + 1) * DIM;
-#pragma unroll
-          for (int d = 0; d < DIM; ++d) out[d] = sg[d];
-          out[DIM] = sg[DIM + 1];
-#pragma unroll
-          for (int v = 0; v <= DIM; ++v) {
-            double s = 0.0;
-#pragma unroll
-            for (int d = 0; d < DIM; ++d) s = fma(ve[v * DIM + d], out[d], s);
-            out[DIM + 1 + v] = s;
-          }
-          if (a.EToB) tag = a.EToB[e * Nfaces + f];
-        }
-#pragma unroll
-        for (int x = 0; x < C::FGS; ++x) fg[ef * C::FGS + x] = out[x];
-        si[EG + ef] = tag;
+      // L2 prefetch of the a6 inputs the consumers will read for this quad
+      if (pt == PT - 1) {
+        const uint32_t bytes = (uint32_t)(nel * Nf * Np * 8);
+        const int64_t off = e0 * Nf * Np;
+        if (a.q_n != nullptr && a.q_n != a.q_in && (a.q_out || a.acc_out)) prefetch_l2(a.q_n + off, bytes);
+        if (a.F0_in != nullptr) prefetch_l2(a.F0_in + off, bytes);
+        if (a.acc_in != nullptr) prefetch_l2(a.acc_in + off, bytes);
       }
-      cp_async_wait_all();
+      load_indices(ql + 1);
+    };
+
+    load_indices(0);
+    if (nq_cta > 0) issue(0);
+    cp_async_commit();
+    for (int ql = 0; ql < nq_cta; ++ql) {
+      const int64_t e0 = ((int64_t)ql * gridDim.x + blockIdx.x) * EG;
+      const int nel = (a.K - e0) < EG ? (int)(a.K - e0) : EG;
+      const int slot = ql % NS;
+      double* qt = sslots + slot * C::slot_doubles;
+      double* gt = qt + C::off_gt;
+      const double* svv = qt + C::off_vv;
+      const double* ssg = qt + C::off_sg;
+      int* si = reinterpret_cast<int*>(qt + C::off_int);
+      const int meta_cur = meta_next;
+      if (ql + 1 < nq_cta) issue(ql + 1);
+      cp_async_commit();
+      if (pt < EG) si[pt] = meta_cur;
+      else if (pt >= 32 && pt < 32 + EG * Nfaces) si[EG + pt - 32] = meta_cur;
+      cp_async_wait_group<1>();   // everything of quad ql has landed (quad ql+1 may still be in flight)
       producer_sync(PT);
-      // ---- a5: upwind flux at my face nodes (eq. 7; reading R7) into the flux tile
+      // ---- a5: upwind flux at my face nodes (eq. 7; reading R7), in place over the gathered q+
 #pragma unroll
       for (int r = 0; r < ROUNDS; ++r) {
-        if (!valid[r]) continue;
         const int fe = task_fe[r], m = task_m[r];
-        const int f = m / Nfp, mm = m - f * Nfp;
+        if (r * PT + pt >= C::NTASK || fe >= nel) continue;
+        const int f = m / Nfp;
         const int n = sfmask[m];
-        double qM[Nf];
+        double qM[Nf], qP[Nf];
 #pragma unroll
-        for (int k = 0; k < Nf; ++k) qM[k] = qt[(fe * Nf + k) * S + n];
-        const double* fd = fg + (fe * Nfaces + f) * C::FGS;
-        double nh[DIM];
+        for (int k = 0; k < Nf; ++k) {
+          qM[k] = qt[(fe * Nf + k) * S + n];
+          qP[k] = gt[(fe * Nf + k) * SG + m];
+        }
+        const double* fd = ssg + (fe * Nfaces + f) * (DIM + 2);
+        double nh[DIM], vG[DIM];
 #pragma unroll
         for (int d = 0; d < DIM; ++d) nh[d] = fd[d];
-        const double Fscale = fd[DIM];
+        const double Fscale = fd[DIM + 1];
+        node_velocity<DIM>(slam + n * (DIM + 1), svv + fe * C::VV, vG);   // P1 mesh velocity at the node (L152, L196)
         double vn = 0.0;
 #pragma unroll
-        for (int v = 0; v <= DIM; ++v) vn = fma(slam[n * (DIM + 1) + v], fd[DIM + 1 + v], vn);
+        for (int d = 0; d < DIM; ++d) vn = fma(vG[d], nh[d], vn);
         const int tag = si[EG + fe * Nfaces + f];
         if (tag == 1) {          // wall moving with the mesh (reading R11)
-          double vG[DIM];
-          node_velocity<DIM>(slam + n * (DIM + 1), a.vvel + (e0 + fe) * (DIM + 1) * DIM, vG);
 #pragma unroll
-          for (int k = 0; k < Nf; ++k) qP[r][k] = qM[k];
+          for (int k = 0; k < Nf; ++k) qP[k] = qM[k];
 #pragma unroll
-          for (int d = 0; d < DIM; ++d) qP[r][1 + d] = 2.0 * qM[0] * vG[d] / cs - qM[1 + d];
+          for (int d = 0; d < DIM; ++d) qP[1 + d] = 2.0 * qM[0] * vG[d] / cs - qM[1 + d];
         } else if (tag != 0) {   // far field
 #pragma unroll
-          for (int k = 0; k < Nf; ++k) qP[r][k] = a.q_inf[k];
+          for (int k = 0; k < Nf; ++k) qP[k] = a.q_inf[k];
         }
         double fl[Nf];
-        upwind_flux<DIM>(qM, qP[r], nh, cs, vn, Fscale, fl);
+        upwind_flux<DIM>(qM, qP, nh, cs, vn, Fscale, fl);
 #pragma unroll
-        for (int k = 0; k < Nf; ++k) gt[(fe * Nf + k) * SG + f * 4 * KF + mm] = fl[k];
+        for (int k = 0; k < Nf; ++k) gt[(fe * Nf + k) * SG + m] = fl[k];
       }
       mbar_arrive(&full[slot]);
     }
@@ -333,7 +297,8 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       const int slot = ql % NS, use = ql / NS;
       const double* qt = sslots + slot * C::slot_doubles;
       const double* gt = qt + C::off_gt;
-      const double* eg = qt + C::off_eg + c * C::EGS;
+      const double* svg = qt + C::off_vg + c * C::VG;
+      const double* svv = qt + C::off_vv + c * C::VV;
       const int* si = reinterpret_cast<const int*>(qt + C::off_int);
       mbar_wait(&full[slot], use & 1);
 
@@ -360,14 +325,15 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       const int nn = n < Np ? n : Np - 1;
       double V[NT][2];
       {
-        double G[DIM * DIM], w[DIM];
+        double G[DIM * DIM], w[DIM], vG[DIM];
 #pragma unroll
-        for (int x = 0; x < DIM * DIM; ++x) G[x] = eg[x];
+        for (int x = 0; x < DIM * DIM; ++x) G[x] = svg[x];
+        node_velocity<DIM>(slam + n * (DIM + 1), svv, vG);   // P1 mesh velocity at the node (L152, L192)
 #pragma unroll
         for (int r = 0; r < DIM; ++r) {
           double s = 0.0;
 #pragma unroll
-          for (int v = 0; v <= DIM; ++v) s = fma(slam[n * (DIM + 1) + v], eg[DIM * DIM + v * DIM + r], s);
+          for (int d = 0; d < DIM; ++d) s = fma(vG[d], G[r * DIM + d], s);
           w[r] = s;   // w_r = v_G . grad(xi_r)
         }
         double st[Nf], qn[Nf], nt[Nf];
@@ -416,11 +382,11 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       }
       // ---- a5: LIFT contraction of the quad's flux tile into the same registers (L103, L196)
 #pragma unroll
-      for (int ks = 0; ks < Nfaces * KF; ++ks) {
+      for (int ks = 0; ks < KFT; ++ks) {
         double bf[NT];
 #pragma unroll
         for (int t = 0; t < NT; ++t) bf[t] = gt[(bcol + 2 * t) * SG + 4 * ks + c];
-        const double af = sAlift[(((ks / KF) * NB + nb) * KF + (ks % KF)) * 32 + lane];
+        const double af = sAlift[(nb * KFT + ks) * 32 + lane];
 #pragma unroll
         for (int t = 0; t < NT; ++t) dmma(V[t][0], V[t][1], af, bf[t]);
       }
