@@ -19,14 +19,19 @@
 #include "alegb_internal.h"
 #include "device_common.cuh"
 
+#ifndef ALEGB_DBG
+#define ALEGB_DBG 0   // timing experiments only: bit mask of phases to skip (results are then wrong)
+#endif
+
 namespace alegb {
 
 namespace pipe {
 
 __host__ __device__ constexpr int stride_pad(int x) {
-  // smallest s >= x with s = 4 (mod 16): B-fragment loads (8 rows x 4 consecutive doubles) are then conflict-free
+  // smallest s >= x with s = 4 (mod 8): the B-fragment loads of a half-warp (4 rows x 4 consecutive doubles) then
+  // fall on 16 distinct 8-byte banks
   int s = x;
-  while (s % 16 != 4) ++s;
+  while (s % 8 != 4) ++s;
   return s;
 }
 
@@ -46,7 +51,7 @@ struct Cfg {
   static constexpr int EG = 4;                 // elements per quad
   static constexpr int PW = 4;                 // producer warps
   static constexpr int CW = 8;                 // consumer warps (12 warps = 3 per SM sub-partition -> 168 registers)
-  static constexpr int NS = 4;                 // slots in the ring
+  static constexpr int NS = 4;                 // slots in the ring (a 5th costs more in L1 capacity than it gains)
   static constexpr int Threads = (PW + CW) * 32;
   static constexpr int PT = PW * 32;           // producer threads
   static constexpr int NTASK = EG * NFN;       // flux tasks per quad
@@ -243,7 +248,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       producer_sync(PT);
       // ---- a5: upwind flux at my face nodes (eq. 7; reading R7), in place over the gathered q+
 #pragma unroll
-      for (int r = 0; r < ROUNDS; ++r) {
+      for (int r = 0; r < ((ALEGB_DBG & 1) ? 0 : ROUNDS); ++r) {
         const int fe = task_fe[r], m = task_m[r];
         if (r * PT + pt >= C::NTASK || fe >= nel) continue;
         const int f = m / Nfp;
@@ -309,7 +314,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
 #pragma unroll
         for (int t = 0; t < NT; ++t) acc[d][t][0] = acc[d][t][1] = 0.0;
 #pragma unroll
-      for (int ks = 0; ks < KS; ++ks) {
+      for (int ks = 0; ks < ((ALEGB_DBG & 2) ? 0 : KS); ++ks) {
         double bf[NT], af[DIM];
 #pragma unroll
         for (int t = 0; t < NT; ++t) bf[t] = qt[(bcol + 2 * t) * S + 4 * ks + c];
@@ -324,7 +329,10 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       const int n = 8 * nb + g;
       const int nn = n < Np ? n : Np - 1;
       double V[NT][2];
-      {
+      if constexpr (ALEGB_DBG & 4) {
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) V[k >> 1][k & 1] = acc[0][k >> 1][k & 1] + acc[1][k >> 1][k & 1] + acc[DIM - 1][k >> 1][k & 1];
+      } else {
         double G[DIM * DIM], w[DIM], vG[DIM];
 #pragma unroll
         for (int x = 0; x < DIM * DIM; ++x) G[x] = svg[x];
@@ -374,7 +382,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
 #pragma unroll
       for (int k = 0; k < Nf; ++k) {
         uq[k] = 0.0; uf[k] = 0.0; ua[k] = 0.0;
-        if (evalid && want_update) {
+        if (evalid && want_update && !(ALEGB_DBG & 16)) {
           if (a.q_n != nullptr) uq[k] = qn_in_tile ? qt[(c * Nf + k) * S + nn] : __ldg(a.q_n + base + k * Np);
           if (a.F0_in != nullptr) uf[k] = __ldg(a.F0_in + base + k * Np);
           if (a.acc_in != nullptr) ua[k] = __ldg(a.acc_in + base + k * Np);
@@ -382,7 +390,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       }
       // ---- a5: LIFT contraction of the quad's flux tile into the same registers (L103, L196)
 #pragma unroll
-      for (int ks = 0; ks < KFT; ++ks) {
+      for (int ks = 0; ks < ((ALEGB_DBG & 8) ? 0 : KFT); ++ks) {
         double bf[NT];
 #pragma unroll
         for (int t = 0; t < NT; ++t) bf[t] = gt[(bcol + 2 * t) * SG + 4 * ks + c];
@@ -393,7 +401,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       // all reads of the slot are done
       mbar_arrive(&empty[slot]);
       // ---- a6: SARK stage update (L132-134), straight from the accumulator registers
-      if (evalid) {
+      if (evalid && (!(ALEGB_DBG & 32) || V[0][0] == 1.2345e300)) {
 #pragma unroll
         for (int k = 0; k < Nf; ++k) {
           const int64_t idx = base + k * Np;
