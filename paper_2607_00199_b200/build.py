@@ -61,9 +61,10 @@ def build(force=False, verbose=False):
         objs.append(o)
     if force or _newer(LIB, objs):
         _run([NVCC, "-shared", "-o", LIB] + objs + ["-lquadmath"], verbose, log)
-    peak_src, peak_bin = os.path.join(CSRC, "fp64_peak.cu"), os.path.join(HERE, "fp64_peak")
-    if os.path.exists(peak_src) and (force or _newer(peak_bin, [peak_src])):
-        _run([NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", peak_bin, peak_src], verbose, log)
+    for tool in ("fp64_peak", "fp64_arbitration"):   # stand-alone microbenchmarks (profiles/r1_fp64_*.md)
+        src, exe = os.path.join(CSRC, tool + ".cu"), os.path.join(HERE, tool)
+        if os.path.exists(src) and (force or _newer(exe, [src])):
+            _run([NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", exe, src], verbose, log)
     with open(os.path.join(OBJ, "build.log"), "a") as f:
         f.write("\n".join(log))
     return LIB
