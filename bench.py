@@ -34,11 +34,14 @@ if ROOT not in sys.path:
 METRIC = "GDOF-stage updates/s (nodes x fields x RK stages)"
 UNIT = "GDOF-stage/s"
 # fp64 pipe peak of one B200: 148 SMs x 64 fp64 FMA lanes per SM and clock x 2 flop x 1.965 GHz (the
-# DFMA/DMMA microbenchmark profiles/fp64_peak_r1.md measured 37.1 TFLOP/s, both instruction kinds share the pipe)
+# DFMA/DMMA microbenchmark profiles/r1_fp64_peak.md measured 37.1 TFLOP/s, both instruction kinds share the pipe)
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 HBM_FALLBACK_GBS = 6650.0
 ALGO_BYTES_PER_DOF_STAGE = 38.0          # 152 B per DOF-step
 POINTWISE_FLOP_PER_DOF_STAGE = 50.0
+# dram__bytes_read.sum + dram__bytes_write.sum of the stage kernel per launch from the committed `ncu --set full`
+# capture (mean over the four stages of a step: 1.79 / 2.93 / 3.48 / 1.82 GB), profiles/r1_v3_pipe_stage_kernel.md
+NCU_DRAM_BYTES_PER_LAUNCH = {4: 2.505e9}
 
 
 def algorithmic_flop_per_dof_stage(dim, Np, Nfp):
@@ -138,6 +141,22 @@ def time_oracle(index, steps, warmup):
     return dof * 4 * steps / wall / 1e9, cores, desc, wall / max(steps, 1) * 1e3, cfg
 
 
+def max_over_ranks(x, world, device):
+    """The slowest rank's time: all-reduce MAX over the job (NCCL on the GPUs, gloo in the CPU tests)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(dof_per_rank, steps, world, elapsed_ms):
+    """Whole-job GDOF-stage/s of `world` independent replicas (weak scaling): all ranks' units / the slowest rank."""
+    return world * dof_per_rank * 4 * steps / (elapsed_ms * 1e-3) / 1e9
+
+
 def run_reference(args, rank):
     if rank != 0:
         return
@@ -227,12 +246,9 @@ def main():
     nprof, prof_ms = ctx.alegb_profile_read()
     ctx.alegb_profile_enable(False)
     clocks = sampler.stop() if sampler else None
-    if world > 1:
-        tmax = torch.tensor([elapsed_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        elapsed_ms = float(tmax.item())
+    elapsed_ms = max_over_ranks(elapsed_ms, world, "cuda")
     finite = bool(torch.isfinite(q).all().item())
-    value = world * dof * 4 * args.steps / (elapsed_ms * 1e-3) / 1e9
+    value = job_throughput(dof, args.steps, world, elapsed_ms)
 
     # ---- end to end through the host-buffer entry point (pinned host state, H2D + step + D2H every step)
     e2e = None
@@ -246,11 +262,8 @@ def main():
             ctx.alegb_step_host(hq, (1 + n) * dt, dt, 1)
         torch.cuda.synchronize()
         el = time.perf_counter() - t0
-        if world > 1:
-            tm = torch.tensor([el], dtype=torch.float64, device="cuda")
-            dist.all_reduce(tm, op=dist.ReduceOp.MAX)
-            el = float(tm.item())
-        e2e = {"value": world * dof * 4 * nsteps_e2e / el / 1e9, "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+        el = max_over_ranks(el, world, "cuda")
+        e2e = {"value": job_throughput(dof, nsteps_e2e, world, el * 1e3), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
                "d2h_bytes_per_step": state_bytes, "steps": nsteps_e2e, "api": "alegb_step_host (pinned host buffer)"}
 
     if rank != 0:
@@ -271,6 +284,10 @@ def main():
            "peak_source": hbm_src, "algorithmic_bytes_per_dof_stage": ALGO_BYTES_PER_DOF_STAGE}
     roofline, other = (alu, hbm) if alu["frac"] >= hbm["frac"] else (hbm, alu)
     roofline = dict(roofline)
+    if args.kernel == 0:
+        roofline["traffic"] = NCU_DRAM_BYTES_PER_LAUNCH.get(args.config)
+        roofline["traffic_unit"] = "bytes per launch (ncu dram read+write, profiles/r1_v3_pipe_stage_kernel.md)"
+        roofline["algorithmic_bytes_per_launch"] = dof * ALGO_BYTES_PER_DOF_STAGE
     roofline.update({"kernel": "alegb stage kernel (fused volume+relaxation+surface+SARK update)",
                      "kernel_ms": kern_ms, "kernel_launches_timed": nprof,
                      "kernel_share_of_step": prof_ms / elapsed_ms if elapsed_ms > 0 else None,
