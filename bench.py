@@ -233,7 +233,11 @@ def main():
     ctx.alegb_step(q, 0.0, dt, args.warmup)
     barrier()
     sampler = ClockSampler(local_rank) if rank == 0 else None
-    ctx.alegb_profile_enable(True)
+    # Large states (the throughput configuration): the library brackets every stage-kernel launch of the timed region
+    # with events (direct launches).  Small, L2-resident states are launch-bound: the timed region replays the
+    # captured step graph (alegb_set_graph) and the stage kernel is timed in a second, direct pass of the same steps.
+    graph_timed = state_bytes < 200e6
+    ctx.alegb_profile_enable(not graph_timed)
     n0 = ctx.alegb_launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -243,6 +247,9 @@ def main():
     barrier()
     elapsed_ms = e0.elapsed_time(e1)
     launches = ctx.alegb_launch_count() - n0
+    if graph_timed:
+        ctx.alegb_profile_enable(True)
+        ctx.alegb_step(q.clone(), args.warmup * dt, dt, args.steps)
     nprof, prof_ms = ctx.alegb_profile_read()
     ctx.alegb_profile_enable(False)
     clocks = sampler.stop() if sampler else None
@@ -291,6 +298,8 @@ def main():
     roofline.update({"kernel": "alegb stage kernel (fused volume+relaxation+surface+SARK update)",
                      "kernel_ms": kern_ms, "kernel_launches_timed": nprof,
                      "kernel_share_of_step": prof_ms / elapsed_ms if elapsed_ms > 0 else None,
+                     "kernel_timed_in": "second pass, direct launches (timed region replays the step graph)"
+                     if graph_timed else "timed region",
                      "other_roof": other})
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -300,7 +309,8 @@ def main():
                        "dt": dt, "parallelism": "replicas x%d (north_star: one GPU, no sharding)" % world,
                        "l2": "state arrays are %.0f MB each (> 126 MB L2), no flush needed" % (state_bytes / 1e6)
                        if state_bytes > 200e6 else "state is L2-resident (%.1f MB); launch-latency bound" % (state_bytes / 1e6),
-                       "state_finite": finite, "kernel": args.kernel},
+                       "state_finite": finite, "kernel": args.kernel,
+                       "launch": "one CUDA graph per step" if graph_timed and args.steps >= 2 else "direct launches"},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
 
     if not args.no_cpu_baseline:

@@ -151,6 +151,12 @@ int64_t alegb_launch_count(const alegb_ctx* ctx);
  * (producer/consumer warps), 3 = warp-per-4-elements DMMA kernel; 2 and 3 return ALEGB_UNSUPPORTED if there is none.
  * All compute the same operator; tests run all of them. */
 int alegb_set_kernel(alegb_ctx* ctx, int kind);
+/* alegb_step with nsteps >= 2 replays ONE captured CUDA graph per step (clock kernel + the a1, a2, a3-a8 launches of
+ * the four stages; stage times t_n + c_i dt are computed on the device with the host loop's IEEE operations, so the
+ * result is bit-identical to nsteps single-step calls).  It removes the per-launch host cost that bounds the small
+ * L2-resident configurations.  on = 0 switches it off (default on).  The graph is not used while
+ * alegb_profile_enable is active.  SURVEY 7 step (8). */
+int alegb_set_graph(alegb_ctx* ctx, int on);
 /* Stage-kernel timing for roofline reports: while enabled, every launch of the fused stage kernel is bracketed by
  * CUDA events on its stream (at most 4096 launches are kept per enable).  alegb_profile_read synchronises the
  * device and returns the number of bracketed launches and the sum of their durations in milliseconds. */

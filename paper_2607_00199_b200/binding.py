@@ -49,6 +49,7 @@ _SIGNATURES = {
     "alegb_last_error": (_c.c_char_p, [_P]),
     "alegb_launch_count": (_c.c_int64, [_P]),
     "alegb_set_kernel": (_c.c_int, [_P, _c.c_int]),
+    "alegb_set_graph": (_c.c_int, [_P, _c.c_int]),
     "alegb_profile_enable": (_c.c_int, [_P, _c.c_int]),
     "alegb_profile_read": (_c.c_int, [_P, _c.POINTER(_c.c_int64), _c.POINTER(_c.c_double)]),
 }
@@ -218,6 +219,9 @@ class Context:
 
     def alegb_set_kernel(self, kind):
         self._check(_lib.alegb_set_kernel(self._h, int(kind)))
+
+    def alegb_set_graph(self, on):
+        self._check(_lib.alegb_set_graph(self._h, int(bool(on))))
 
     def alegb_profile_enable(self, on):
         self._check(_lib.alegb_profile_enable(self._h, int(bool(on))))

@@ -42,6 +42,14 @@ struct alegb_ctx {
   bool profiling = false;
   std::vector<cudaEvent_t> prof_events;  // pairs (start, stop), created on demand
   size_t prof_used = 0;
+  // one SARK4 step captured as a CUDA graph (alegb_step with nsteps >= 2): stage times live on the device
+  bool use_graph = true;
+  uint64_t config_version = 0;        // bumped by every call that changes what a step launches
+  cudaStream_t capture_stream = nullptr;
+  cudaGraphExec_t step_graph = nullptr;
+  struct { double* d_q; double dt; uint64_t version; int64_t launches; } graph_key{nullptr, 0, 0, 0};
+  double* d_clock = nullptr;          // {t0, dt, stage times[4]} of the current run of steps
+  long long* d_step_counter = nullptr;
   std::string err;
 };
 
@@ -88,15 +96,16 @@ void free_mesh(alegb_ctx* ctx) {
   dev_free(ctx->d_AUX); dev_free(ctx->d_AUXS); dev_free(ctx->d_AUXACC);
   ctx->mesh_ready = false;
   ctx->K = ctx->Nverts = ctx->Kpml = 0;
+  ctx->config_version++;
 }
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 // a1 + a2 at time t into the context's geometry arrays
-int update_geometry(alegb_ctx* ctx, double t, cudaStream_t s) {
+int update_geometry(alegb_ctx* ctx, double t, cudaStream_t s, const double* t_dev = nullptr) {
   const int dim = ctx->ref.dim;
   if (ctx->motion.kind != ALEGB_MOTION_USER) {
-    CU(launch_vertex_motion(dim, ctx->Nverts, ctx->d_X0, ctx->motion, t, ctx->d_xv, ctx->d_vv, s));
+    CU(launch_vertex_motion(dim, ctx->Nverts, ctx->d_X0, ctx->motion, t, t_dev, ctx->d_xv, ctx->d_vv, s));
     ctx->launches++;
   }
   CU(launch_geometry(dim, ctx->K, ctx->d_EToV, ctx->d_xv, ctx->d_vv, ctx->d_vgeo, ctx->d_sgeo, ctx->d_vvel, s));
@@ -160,7 +169,8 @@ int timed_stage(alegb_ctx* ctx, const StageArgs& a, cudaStream_t s) {
 
 // One SARK4 step.  q_n: state at t0 (read only); outs[i]: where stage state i+1 is written
 // (outs[3] = q_{n+1}, may alias q_n).
-int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t0, double dt, cudaStream_t s) {
+int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t0, double dt, cudaStream_t s,
+              const double* t_dev = nullptr) {
   const int dim = ctx->ref.dim, N = ctx->ref.N, Nf = ctx->Nf;
   const double gamma = -dt * ctx->invtau;  // L144
   double as[6], bs[4], a0[6], b0[4];
@@ -180,7 +190,7 @@ int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t
   const bool pml = ctx->Kpml > 0;
   for (int i = 0; i < 4; ++i) {
     const double ti = t0 + cstage[i] * dt;
-    int rc = update_geometry(ctx, ti, s);
+    int rc = update_geometry(ctx, ti, s, t_dev ? t_dev + i : nullptr);
     if (rc != ALEGB_OK) return rc;
     StageArgs a;
     fill_common(ctx, a);
@@ -229,6 +239,52 @@ int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t
       ctx->launches++;
     }
   }
+  return ALEGB_OK;
+}
+
+void drop_step_graph(alegb_ctx* ctx) {
+  if (ctx->step_graph) cudaGraphExecDestroy(ctx->step_graph);
+  ctx->step_graph = nullptr;
+}
+
+// nsteps SARK4 steps as nsteps launches of ONE captured graph (clock kernel + the 12-16 launches of a step): removes
+// the per-launch host cost that bounds the small, L2-resident configurations.  The graph is captured on a stream of
+// the library's own (the caller's may be the legacy default stream, which cannot be captured) and launched on the
+// caller's stream; it is rebuilt when the state pointer, dt or anything a step launches changes (t0 lives on the device).
+int step_graph_launch(alegb_ctx* ctx, double* d_q, double* const outs[4], double t0, double dt, int nsteps, cudaStream_t s) {
+  if (!ctx->capture_stream) CU(cudaStreamCreateWithFlags(&ctx->capture_stream, cudaStreamNonBlocking));
+  if (!ctx->d_clock) {
+    CU(dev_alloc(ctx, &ctx->d_clock, 6));
+    CU(dev_alloc(ctx, &ctx->d_step_counter, 1));
+  }
+  auto& key = ctx->graph_key;
+  if (!ctx->step_graph || key.d_q != d_q || key.dt != dt || key.version != ctx->config_version) {
+    drop_step_graph(ctx);
+    const int64_t before = ctx->launches;
+    cudaGraph_t graph = nullptr;
+    if (cudaStreamBeginCapture(ctx->capture_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+      cudaGetLastError();
+      return ALEGB_UNSUPPORTED;
+    }
+    int rc = ALEGB_OK;
+    if (launch_step_clock(ctx->d_clock, ctx->d_step_counter, ctx->capture_stream) != cudaSuccess) rc = ALEGB_CUDA_ERROR;
+    if (rc == ALEGB_OK) rc = sark_step(ctx, d_q, outs, t0, dt, ctx->capture_stream, ctx->d_clock + 2);
+    cudaError_t e = cudaStreamEndCapture(ctx->capture_stream, &graph);
+    key.launches = ctx->launches - before + 1;
+    ctx->launches = before;
+    if (rc != ALEGB_OK || e != cudaSuccess || graph == nullptr) {
+      if (graph) cudaGraphDestroy(graph);
+      cudaGetLastError();
+      return rc != ALEGB_OK ? rc : ALEGB_UNSUPPORTED;
+    }
+    e = cudaGraphInstantiate(&ctx->step_graph, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) { ctx->step_graph = nullptr; cudaGetLastError(); return ALEGB_UNSUPPORTED; }
+    key.d_q = d_q; key.dt = dt; key.version = ctx->config_version;
+  }
+  CU(launch_step_clock_set(ctx->d_clock, ctx->d_step_counter, t0, dt, s));
+  for (int n = 0; n < nsteps; ++n) CU(cudaGraphLaunch(ctx->step_graph, s));
+  ctx->launches += key.launches * nsteps + 1;
   return ALEGB_OK;
 }
 
@@ -320,6 +376,9 @@ int alegb_destroy(alegb_ctx* ctx) {
     cudaDeviceSynchronize();
   }
   free_mesh(ctx);
+  drop_step_graph(ctx);
+  if (ctx->capture_stream) cudaStreamDestroy(ctx->capture_stream);
+  dev_free(ctx->d_clock); dev_free(ctx->d_step_counter);
   for (cudaEvent_t ev : ctx->prof_events) cudaEventDestroy(ev);
   dev_free(ctx->d_Dt); dev_free(ctx->d_LIFTt); dev_free(ctx->d_lam); dev_free(ctx->d_fmask);
   dev_free(ctx->d_Avol); dev_free(ctx->d_Alift); dev_free(ctx->d_AliftP);
@@ -422,6 +481,7 @@ int alegb_set_params(alegb_ctx* ctx, double RT, double tau, const double* q_inf)
   for (int k = 0; k < kMaxFields; ++k) ctx->q_inf[k] = 0.0;
   if (q_inf) for (int k = 0; k < ctx->Nf; ++k) ctx->q_inf[k] = q_inf[k];
   ctx->params_ready = true;
+  ctx->config_version++;
   return ALEGB_OK;
 }
 
@@ -444,6 +504,7 @@ int alegb_set_motion(alegb_ctx* ctx, int kind, const double* params, int nparams
   }
   ctx->motion.kind = kind; ctx->motion.nparams = need;
   for (int i = 0; i < 16; ++i) ctx->motion.p[i] = i < need ? params[i] : 0.0;
+  ctx->config_version++;
   return ALEGB_OK;
 }
 
@@ -458,6 +519,7 @@ int alegb_set_motion_user(alegb_ctx* ctx, const double* d_xv, const double* d_vv
   CU(cudaMemcpyAsync(ctx->d_vv, d_vv, bytes, cudaMemcpyDeviceToDevice, 0));
   CU(cudaStreamSynchronize(0));
   ctx->motion.kind = ALEGB_MOTION_USER;
+  ctx->config_version++;
   return ALEGB_OK;
 }
 
@@ -497,6 +559,10 @@ int alegb_step(alegb_ctx* ctx, double* d_q, double t0, double dt, int nsteps, vo
   if (!aligned16(d_q)) return fail(ctx, ALEGB_INVALID_ARG, "field pointers must be 16-byte aligned");
   cudaStream_t s = (cudaStream_t)stream;
   double* outs[4] = {ctx->d_Q1, ctx->d_Q2, ctx->d_Q1, d_q};
+  if (ctx->use_graph && !ctx->profiling && nsteps >= 2) {
+    rc = step_graph_launch(ctx, d_q, outs, t0, dt, nsteps, s);
+    if (rc != ALEGB_UNSUPPORTED) return rc;   // UNSUPPORTED: capture not possible here, launch directly instead
+  }
   for (int n = 0; n < nsteps; ++n) {
     rc = sark_step(ctx, d_q, outs, t0 + n * dt, dt, s);
     if (rc != ALEGB_OK) return rc;
@@ -639,6 +705,13 @@ int alegb_set_kernel(alegb_ctx* ctx, int kind) {
   if (kind == 2 && !ctx->pipe_ok) return fail(ctx, ALEGB_UNSUPPORTED, "no pipelined DMMA stage kernel for this (dim, N)");
   if (kind == 3 && !ctx->mma_ok) return fail(ctx, ALEGB_UNSUPPORTED, "no DMMA stage kernel for this (dim, N)");
   ctx->kernel_mode = kind;
+  ctx->config_version++;
+  return ALEGB_OK;
+}
+
+int alegb_set_graph(alegb_ctx* ctx, int on) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  ctx->use_graph = on != 0;
   return ALEGB_OK;
 }
 

@@ -80,8 +80,12 @@ struct MotionArgs {
 };
 
 // kernel launchers (kernels.cu); return cudaGetLastError()
-cudaError_t launch_vertex_motion(int dim, int64_t Nverts, const double* X0, const MotionArgs& m, double t, double* xv,
-                                 double* vv, cudaStream_t s);
+// t_dev != NULL: the stage time is read from the device (graph-captured steps) and t is ignored
+cudaError_t launch_vertex_motion(int dim, int64_t Nverts, const double* X0, const MotionArgs& m, double t,
+                                 const double* t_dev, double* xv, double* vv, cudaStream_t s);
+// clock = {t0, dt, stage times[4]} on the device; _set starts a run of steps, the other advances to the next step
+cudaError_t launch_step_clock(double* clock, long long* counter, cudaStream_t s);
+cudaError_t launch_step_clock_set(double* clock, long long* counter, double t0, double dt, cudaStream_t s);
 cudaError_t launch_geometry(int dim, int64_t K, const int32_t* EToV, const double* xv, const double* vv, double* vgeo,
                             double* sgeo, double* vvel, cudaStream_t s);
 // returns cudaErrorInvalidValue if (dim, N) has no compiled kernel

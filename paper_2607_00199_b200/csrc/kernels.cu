@@ -17,9 +17,11 @@ namespace alegb {
 // a1: vertex motion.  One thread per vertex.
 template <int DIM>
 __global__ void vertex_motion_kernel(int64_t Nverts, const double* __restrict__ X0, MotionArgs m, double t,
-                                     double* __restrict__ xv, double* __restrict__ vv) {
+                                     const double* __restrict__ t_dev, double* __restrict__ xv,
+                                     double* __restrict__ vv) {
   int64_t v = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (v >= Nverts) return;
+  if (t_dev != nullptr) t = *t_dev;   // stage time kept on the device (graph-captured steps)
   double X[DIM], disp[DIM], vel[DIM];
 #pragma unroll
   for (int d = 0; d < DIM; ++d) { X[d] = X0[v * DIM + d]; disp[d] = 0.0; vel[d] = 0.0; }
@@ -82,12 +84,37 @@ __global__ void vertex_motion_kernel(int64_t Nverts, const double* __restrict__ 
   for (int d = 0; d < DIM; ++d) { xv[v * DIM + d] = X[d] + disp[d]; vv[v * DIM + d] = vel[d]; }
 }
 
-cudaError_t launch_vertex_motion(int dim, int64_t Nverts, const double* X0, const MotionArgs& m, double t, double* xv,
-                                 double* vv, cudaStream_t s) {
+cudaError_t launch_vertex_motion(int dim, int64_t Nverts, const double* X0, const MotionArgs& m, double t,
+                                 const double* t_dev, double* xv, double* vv, cudaStream_t s) {
   if (Nverts == 0) return cudaSuccess;
   int nb = (int)((Nverts + 255) / 256);
-  if (dim == 2) vertex_motion_kernel<2><<<nb, 256, 0, s>>>(Nverts, X0, m, t, xv, vv);
-  else vertex_motion_kernel<3><<<nb, 256, 0, s>>>(Nverts, X0, m, t, xv, vv);
+  if (dim == 2) vertex_motion_kernel<2><<<nb, 256, 0, s>>>(Nverts, X0, m, t, t_dev, xv, vv);
+  else vertex_motion_kernel<3><<<nb, 256, 0, s>>>(Nverts, X0, m, t, t_dev, xv, vv);
+  return cudaGetLastError();
+}
+
+// Stage times of the next step on the device, for graph-captured steps.  clock = {t0, dt, times[4]}:
+// n = *counter, t_n = t0 + n dt, times[i] = t_n + c_i dt (c = 0, 1/2, 1/2, 1; L126), then *counter = n + 1.  Plain IEEE
+// multiply and add in the same order as the host loop of alegb_step, so both paths see bit-identical stage times.
+__global__ void step_clock_kernel(double* clock, long long* counter) {
+  const long long n = *counter;
+  const double t0 = clock[0], dt = clock[1];
+  const double tn = __dadd_rn(t0, __dmul_rn((double)n, dt));
+  const double cst[4] = {0.0, 0.5, 0.5, 1.0};
+  for (int i = 0; i < 4; ++i) clock[2 + i] = __dadd_rn(tn, __dmul_rn(cst[i], dt));
+  *counter = n + 1;
+}
+__global__ void step_clock_set_kernel(double* clock, long long* counter, double t0, double dt) {
+  clock[0] = t0;
+  clock[1] = dt;
+  *counter = 0;
+}
+cudaError_t launch_step_clock(double* clock, long long* counter, cudaStream_t s) {
+  step_clock_kernel<<<1, 1, 0, s>>>(clock, counter);
+  return cudaGetLastError();
+}
+cudaError_t launch_step_clock_set(double* clock, long long* counter, double t0, double dt, cudaStream_t s) {
+  step_clock_set_kernel<<<1, 1, 0, s>>>(clock, counter, t0, dt);
   return cudaGetLastError();
 }
 

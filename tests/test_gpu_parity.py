@@ -335,6 +335,47 @@ def test_step_host_roundtrip(refs, B):
     ctx.close()
 
 
+@pytest.mark.parametrize("name", ["cfg1", "cfg3", "cfg4"])
+def test_graph_replay_is_bit_identical_to_direct_launches(name, refs, B):
+    """alegb_step(nsteps >= 2) replays one captured CUDA graph per step with the stage times kept on the device
+    (include/alegb.h: alegb_set_graph).  Same kernels, same arguments, same stage times => identical bits as the
+    direct launches; also after t0 changes (no re-capture), after set_motion (re-capture) and on a user stream."""
+    ref, cfg = make_case(name, refs)
+    ctx = B.context_from_config(cfg)
+    q = perturbed(cfg)
+    dt = cfg["dt"]
+
+    def run(graph, t0, nsteps, stream=None):
+        ctx.alegb_set_graph(graph)
+        ctx.alegb_pml_reset()
+        dq = dev(q)
+        n0 = ctx.alegb_launch_count()
+        if stream is None:
+            ctx.alegb_step(dq, t0, dt, nsteps)
+        else:
+            with torch.cuda.stream(stream):
+                ctx.alegb_step(dq, t0, dt, nsteps)
+            stream.synchronize()
+        torch.cuda.synchronize()
+        return dq.cpu().numpy(), ctx.alegb_launch_count() - n0
+
+    direct, nd = run(False, 0.3, 5)
+    replay, ng = run(True, 0.3, 5)
+    assert np.array_equal(direct, replay)
+    assert ng == nd + 5 + 1                      # one clock kernel per step + one clock set per call
+    direct2, _ = run(False, 0.7, 3)
+    replay2, _ = run(True, 0.7, 3)               # same graph, new t0 on the device
+    assert np.array_equal(direct2, replay2) and not np.array_equal(direct2, direct)
+    replay3, _ = run(True, 0.3, 5, torch.cuda.Stream())
+    assert np.array_equal(direct, replay3)
+    if cfg["motion_kind"] != 0:                  # changing the motion law invalidates the captured graph
+        ctx.alegb_set_motion(0, [])
+        still, _ = run(True, 0.3, 5)
+        ref_still, _ = run(False, 0.3, 5)
+        assert np.array_equal(still, ref_still) and not np.array_equal(still, direct)
+    ctx.close()
+
+
 def test_full_size_throughput_config_sampled(refs, B):
     """BASELINE.json configs[3] at full size (196,608 tets, N = 4), the launch configuration bench.py times.
     The oracle computes a sample of elements one patch at a time (helpers.submesh): F needs the face neighbours,
