@@ -26,6 +26,7 @@ struct alegb_ctx {
   int32_t* d_fmask = nullptr;
   bool mma_ok = false;   // a warp-per-quad DMMA stage kernel exists for (dim, N)
   bool pipe_ok = false;  // a pipelined DMMA stage kernel exists for (dim, N)
+  bool pml_mma_ok = false;  // a DMMA kernel for the absorbing layer's auxiliary fields exists for (dim, N)
   int kernel_mode = 0;   // 0 auto (pipelined DMMA, else DMMA, else generic), 1 generic, 2 pipelined DMMA, 3 warp-per-quad DMMA
   // device: mesh
   double *d_X0 = nullptr, *d_xv = nullptr, *d_vv = nullptr;
@@ -130,8 +131,14 @@ void fill_common(const alegb_ctx* ctx, PmlArgs& a) {
   a.vgeo = ctx->d_vgeo; a.sgeo = ctx->d_sgeo; a.vvel = ctx->d_vvel;
   a.vmapP = ctx->d_vmapP; a.EToB = ctx->d_EToB;
   a.Dt_ops = ctx->d_Dt; a.LIFTt = ctx->d_LIFTt; a.lam = ctx->d_lam; a.fmask = ctx->d_fmask;
+  a.Avol = ctx->d_Avol; a.AliftP = ctx->d_AliftP;
   a.c = ctx->c;
   for (int k = 0; k < kMaxFields; ++k) a.q_inf[k] = ctx->q_inf[k];
+}
+// a8: the DMMA kernel unless the generic kernels were asked for (alegb_set_kernel(1)) or (dim, N) has none
+cudaError_t launch_pml_any(const alegb_ctx* ctx, const PmlArgs& p, cudaStream_t s) {
+  if (ctx->pml_mma_ok && ctx->kernel_mode != 1) return launch_pml_mma(ctx->ref.dim, ctx->ref.N, p, ctx->num_sms, s);
+  return launch_pml(ctx->ref.dim, ctx->ref.N, p, ctx->num_sms, s);
 }
 
 int check_ready(alegb_ctx* ctx) {
@@ -235,7 +242,7 @@ int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t
       } else {
         p.acc_in = ctx->d_AUXACC; p.aux_out = ctx->d_AUX; p.cx_acc = 1.0; p.cx_g = dt * (1.0 / 6.0);
       }
-      CU(launch_pml(dim, N, p, ctx->num_sms, s));
+      CU(launch_pml_any(ctx, p, s));
       ctx->launches++;
     }
   }
@@ -327,6 +334,8 @@ int alegb_create(alegb_ctx** out, int dim, int N, int cuda_device) {
   MmaLayout L{};
   ctx->mma_ok = mma_layout(dim, N, L) && configure_stage_mma(dim, N) == cudaSuccess;
   ctx->pipe_ok = ctx->mma_ok && configure_stage_pipe(dim, N) == cudaSuccess;
+  ctx->pml_mma_ok = ctx->mma_ok && configure_pml_mma(dim, N) == cudaSuccess;
+  cudaGetLastError();
   if (ctx->mma_ok) {
     std::vector<double> Av((size_t)dim * L.NB * L.KS * 32, 0.0), Al((size_t)r.Nfaces * L.NB * L.KF * 32, 0.0);
     for (int a = 0; a < dim; ++a)
@@ -542,7 +551,7 @@ int alegb_rhs_pml(alegb_ctx* ctx, double t, const double* d_q, const double* d_a
     PmlArgs p;
     fill_common(ctx, p);
     p.q_in = d_q; p.aux_in = a.aux; p.G_out = d_Faux;
-    CU(launch_pml(ctx->ref.dim, ctx->ref.N, p, ctx->num_sms, s));
+    CU(launch_pml_any(ctx, p, s));
     ctx->launches++;
   }
   return ALEGB_OK;

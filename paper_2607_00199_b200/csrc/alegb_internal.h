@@ -63,6 +63,7 @@ struct PmlArgs {
   const double* vgeo; const double* sgeo; const double* vvel;
   const int32_t* vmapP; const int8_t* EToB;
   const double* Dt_ops; const double* LIFTt; const double* lam; const int32_t* fmask;
+  const double* Avol; const double* AliftP;   // DMMA path (pml_mma.cu): operator fragments as in StageArgs
   double c;
   double q_inf[kMaxFields];
   const double* q_in;
@@ -98,6 +99,10 @@ struct MmaLayout { int NB, KS, KF; };               // node blocks, k-steps of t
 bool mma_layout(int dim, int N, MmaLayout& L);       // false if (dim, N) has no DMMA kernel
 cudaError_t configure_stage_mma(int dim, int N);
 cudaError_t launch_stage_mma(int dim, int N, const StageArgs& a, int num_sms, cudaStream_t s);
+
+// tensor-core kernel of the absorbing layer's auxiliary fields, pml_mma.cu
+cudaError_t configure_pml_mma(int dim, int N);        // cudaErrorInvalidValue if (dim, N) has no such kernel
+cudaError_t launch_pml_mma(int dim, int N, const PmlArgs& a, int num_sms, cudaStream_t s);
 
 // pipelined tensor-core stage kernel (producer / consumer warps), stage_pipe.cu; same operator fragments
 cudaError_t configure_stage_pipe(int dim, int N);     // cudaErrorInvalidValue if (dim, N) has no such kernel
