@@ -377,15 +377,29 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
             V[k >> 1][k & 1] -= sig * a.aux[(((int64_t)pml * DIM + d) * Nf + k) * Np + nn];
         }
       }
-      // ---- a6 inputs, requested before the LIFT contraction so that their latency hides behind it
+      // ---- a6 inputs, requested before the LIFT contraction so that their latency hides behind it (one uniform
+      //      branch per array, straight-line loads with immediate offsets inside)
       double uq[Nf], uf[Nf], ua[Nf];
 #pragma unroll
-      for (int k = 0; k < Nf; ++k) {
-        uq[k] = 0.0; uf[k] = 0.0; ua[k] = 0.0;
-        if (evalid && want_update && !(ALEGB_DBG & 16)) {
-          if (a.q_n != nullptr) uq[k] = qn_in_tile ? qt[(c * Nf + k) * S + nn] : __ldg(a.q_n + base + k * Np);
-          if (a.F0_in != nullptr) uf[k] = __ldg(a.F0_in + base + k * Np);
-          if (a.acc_in != nullptr) ua[k] = __ldg(a.acc_in + base + k * Np);
+      for (int k = 0; k < Nf; ++k) { uq[k] = 0.0; uf[k] = 0.0; ua[k] = 0.0; }
+      if (evalid && want_update && !(ALEGB_DBG & 16)) {
+        if (qn_in_tile) {
+#pragma unroll
+          for (int k = 0; k < Nf; ++k) uq[k] = qt[(c * Nf + k) * S + nn];
+        } else if (a.q_n != nullptr) {
+          const double* pq = a.q_n + base;
+#pragma unroll
+          for (int k = 0; k < Nf; ++k) uq[k] = __ldg(pq + k * Np);
+        }
+        if (a.F0_in != nullptr) {
+          const double* pf = a.F0_in + base;
+#pragma unroll
+          for (int k = 0; k < Nf; ++k) uf[k] = __ldg(pf + k * Np);
+        }
+        if (a.acc_in != nullptr) {
+          const double* pa = a.acc_in + base;
+#pragma unroll
+          for (int k = 0; k < Nf; ++k) ua[k] = __ldg(pa + k * Np);
         }
       }
       // ---- a5: LIFT contraction of the quad's flux tile into the same registers (L103, L196)
@@ -400,24 +414,31 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       }
       // all reads of the slot are done
       mbar_arrive(&empty[slot]);
-      // ---- a6: SARK stage update (L132-134), straight from the accumulator registers
+      // ---- a6: SARK stage update (L132-134), straight from the accumulator registers; one uniform branch per output
       if (evalid && (!(ALEGB_DBG & 32) || V[0][0] == 1.2345e300)) {
+        if (a.F_out != nullptr) {
+          double* of = a.F_out + base;
 #pragma unroll
-        for (int k = 0; k < Nf; ++k) {
-          const int64_t idx = base + k * Np;
-          const double F = V[k >> 1][k & 1];
-          if (a.F_out) a.F_out[idx] = F;
-          if (a.q_out) {
+          for (int k = 0; k < Nf; ++k) of[k * Np] = V[k >> 1][k & 1];
+        }
+        if (a.q_out != nullptr) {
+          double* oq = a.q_out + base;
+#pragma unroll
+          for (int k = 0; k < Nf; ++k) {
             double v = a.coef.cq_n[k] * uq[k];
             v = fma(a.coef.cq_f0[k], uf[k], v);
             v = fma(a.coef.cq_acc, ua[k], v);
-            a.q_out[idx] = fma(a.coef.cq_f[k], F, v);
+            oq[k * Np] = fma(a.coef.cq_f[k], V[k >> 1][k & 1], v);
           }
-          if (a.acc_out) {
+        }
+        if (a.acc_out != nullptr) {
+          double* oa = a.acc_out + base;
+#pragma unroll
+          for (int k = 0; k < Nf; ++k) {
             double v = a.coef.ca_n[k] * uq[k];
             v = fma(a.coef.ca_f0[k], uf[k], v);
             v = fma(a.coef.ca_acc, ua[k], v);
-            a.acc_out[idx] = fma(a.coef.ca_f[k], F, v);
+            oa[k * Np] = fma(a.coef.ca_f[k], V[k >> 1][k & 1], v);
           }
         }
       }
