@@ -15,6 +15,8 @@ constexpr int kMaxFields = 10;
 // Per-field coefficients of one fused stage (PAPER.md:L132-134 written as two linear combinations):
 //   q_out   = cq_n  q_n + cq_f0 F0 + cq_acc acc_in + cq_f F
 //   acc_out = ca_n  q_n + ca_f0 F0 + ca_acc acc_in + ca_f F
+// The per-field values depend on the field k only through k <= dim (lambda = 0) or k > dim (lambda = 1/tau, L115):
+// stage_pipe.cu reads entries [0] and [dim + 1] only.
 // F is the operator of eq. 9 evaluated on q_in at the stage time.  A NULL output pointer skips that output; inputs
 // whose coefficients are all zero are not read.
 struct StageCoef {

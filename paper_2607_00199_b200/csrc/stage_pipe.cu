@@ -421,26 +421,30 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
 #pragma unroll
           for (int k = 0; k < Nf; ++k) of[k * Np] = V[k >> 1][k & 1];
         }
-        if (a.q_out != nullptr) {
-          double* oq = a.q_out + base;
+        // the coefficients depend on the field only through stiff / non-stiff (StageCoef): two values each
+        const bool hf = a.F0_in != nullptr, ha = a.acc_in != nullptr;
+        auto combine = [&](const double* cn, const double* cf0, double cacc, const double* cf, double* out) {
+          const double n0 = cn[0], n1 = cn[DIM + 1], f00 = cf0[0], f01 = cf0[DIM + 1], g0 = cf[0], g1 = cf[DIM + 1];
+          if (hf && ha) {
 #pragma unroll
-          for (int k = 0; k < Nf; ++k) {
-            double v = a.coef.cq_n[k] * uq[k];
-            v = fma(a.coef.cq_f0[k], uf[k], v);
-            v = fma(a.coef.cq_acc, ua[k], v);
-            oq[k * Np] = fma(a.coef.cq_f[k], V[k >> 1][k & 1], v);
-          }
-        }
-        if (a.acc_out != nullptr) {
-          double* oa = a.acc_out + base;
+            for (int k = 0; k < Nf; ++k)
+              out[k * Np] = fma(k > DIM ? g1 : g0, V[k >> 1][k & 1],
+                                fma(cacc, ua[k], fma(k > DIM ? f01 : f00, uf[k], (k > DIM ? n1 : n0) * uq[k])));
+          } else if (hf) {
 #pragma unroll
-          for (int k = 0; k < Nf; ++k) {
-            double v = a.coef.ca_n[k] * uq[k];
-            v = fma(a.coef.ca_f0[k], uf[k], v);
-            v = fma(a.coef.ca_acc, ua[k], v);
-            oa[k * Np] = fma(a.coef.ca_f[k], V[k >> 1][k & 1], v);
+            for (int k = 0; k < Nf; ++k)
+              out[k * Np] = fma(k > DIM ? g1 : g0, V[k >> 1][k & 1], fma(k > DIM ? f01 : f00, uf[k], (k > DIM ? n1 : n0) * uq[k]));
+          } else if (ha) {
+#pragma unroll
+            for (int k = 0; k < Nf; ++k)
+              out[k * Np] = fma(k > DIM ? g1 : g0, V[k >> 1][k & 1], fma(cacc, ua[k], (k > DIM ? n1 : n0) * uq[k]));
+          } else {
+#pragma unroll
+            for (int k = 0; k < Nf; ++k) out[k * Np] = fma(k > DIM ? g1 : g0, V[k >> 1][k & 1], (k > DIM ? n1 : n0) * uq[k]);
           }
-        }
+        };
+        if (a.q_out != nullptr) combine(a.coef.cq_n, a.coef.cq_f0, a.coef.cq_acc, a.coef.cq_f, a.q_out + base);
+        if (a.acc_out != nullptr) combine(a.coef.ca_n, a.coef.ca_f0, a.coef.ca_acc, a.coef.ca_f, a.acc_out + base);
       }
     }
   }
