@@ -51,9 +51,24 @@ struct Cfg {
   static constexpr int EG = 4;                 // elements per quad
   static constexpr int PW = 4;                 // producer warps
   static constexpr int CW = 8;                 // consumer warps (12 warps = 3 per SM sub-partition -> 168 registers)
-  static constexpr int NS = 4;                 // slots in the ring (a 5th costs more in L1 capacity than it gains)
+  // Producer groups.  3-D: the four producer warps work on ONE quad together (a quad is 1400 doubles of q and 240
+  // flux tasks at N=4) and the ring has 4 slots (a 5th costs more in L1 capacity than it gains).  2-D: a quad is a
+  // few hundred doubles and 36 DMMA per item, the per-quad latency chain of the producers (indices -> copies ->
+  // barrier -> flux) is what bounds the kernel (profiles/r1_v12_cfg3_stage_kernel.md), so every producer warp
+  // streams quads of its own (warp w takes quads w, w+4, ...) into a deeper ring.
+#ifdef ALEGB_PG
+  static constexpr int PG = ALEGB_PG;
+#else
+  static constexpr int PG = DIM == 2 ? 32 : PW * 32;   // threads of one producer group
+#endif
+#ifdef ALEGB_NS
+  static constexpr int NS = ALEGB_NS;
+#else
+  static constexpr int NS = PG == 32 ? 12 : 4;         // slots in the ring
+#endif
+  static constexpr int NG = PW * 32 / PG;      // producer groups
   static constexpr int Threads = (PW + CW) * 32;
-  static constexpr int PT = PW * 32;           // producer threads
+  static constexpr int PT = PG;                // threads producing one quad
   static constexpr int NTASK = EG * NFN;       // flux tasks per quad
   static constexpr int ROUNDS = (NTASK + PT - 1) / PT;
   // per-element geometry records, copied raw from the geometry kernel's arrays
@@ -108,8 +123,10 @@ __device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.w
 __device__ __forceinline__ void prefetch_l2(const void* p, uint32_t bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void producer_sync(int nthreads) {
-  asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
+template <int NTHREADS>
+__device__ __forceinline__ void producer_sync(int group) {   // the threads of one producer group
+  if constexpr (NTHREADS == 32) __syncwarp();
+  else asm volatile("bar.sync %0, %1;" ::"r"(1 + group), "n"(NTHREADS) : "memory");
 }
 
 }  // namespace pipe
@@ -156,8 +173,9 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
   if (warp < C::PW) {
     // =================================================================================================== producers
     // Every global read of a quad is asynchronous (cp.async straight into its slot) and issued one quad ahead of
-    // the flux arithmetic, so the producers never sit on a load: iteration ql issues quad ql+1, then computes quad ql.
-    const int pt = tid;
+    // the flux arithmetic, so the producers never sit on a load: a group's iteration issues its next quad, then
+    // computes the current one.
+    const int pt = tid % PT, grp = tid / PT;   // thread within its producer group, group
     constexpr int ROUNDS = C::ROUNDS;
     int task_fe[ROUNDS], task_m[ROUNDS];
 #pragma unroll
@@ -167,7 +185,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       task_m[r] = task - task_fe[r] * NFN;
     }
     int idx_next[ROUNDS];   // vmapP entries of my face nodes in the quad that is issued next
-    int meta_next = 0;      // pml index (threads < EG) / boundary tag (threads 32 .. 32+EG*Nfaces) of that quad
+    int meta_next = 0;      // pml index (threads < EG) / boundary tag (threads EG .. EG+EG*Nfaces) of that quad
 
     auto load_indices = [&](int ql) {
       const int64_t e0 = ((int64_t)ql * gridDim.x + blockIdx.x) * EG;
@@ -212,8 +230,8 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       meta_next = pt < EG ? -1 : 0;
       if (pt < EG) {
         if (pt < nel && a.pml_index != nullptr && a.aux != nullptr) meta_next = __ldg(a.pml_index + e0 + pt);
-      } else if (pt >= 32 && pt < 32 + EG * Nfaces) {
-        const int ef = pt - 32;
+      } else if (pt < EG + EG * Nfaces) {
+        const int ef = pt - EG;
         if (ef < nel * Nfaces && a.EToB != nullptr) meta_next = a.EToB[e0 * Nfaces + ef];
       }
       // L2 prefetch of the a6 inputs the consumers will read for this quad
@@ -224,13 +242,13 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
         if (a.F0_in != nullptr) prefetch_l2(a.F0_in + off, bytes);
         if (a.acc_in != nullptr) prefetch_l2(a.acc_in + off, bytes);
       }
-      load_indices(ql + 1);
+      load_indices(ql + C::NG);
     };
 
-    load_indices(0);
-    if (nq_cta > 0) issue(0);
+    load_indices(grp);
+    if (grp < nq_cta) issue(grp);
     cp_async_commit();
-    for (int ql = 0; ql < nq_cta; ++ql) {
+    for (int ql = grp; ql < nq_cta; ql += C::NG) {
       const int64_t e0 = ((int64_t)ql * gridDim.x + blockIdx.x) * EG;
       const int nel = (a.K - e0) < EG ? (int)(a.K - e0) : EG;
       const int slot = ql % NS;
@@ -240,12 +258,11 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       const double* ssg = qt + C::off_sg;
       int* si = reinterpret_cast<int*>(qt + C::off_int);
       const int meta_cur = meta_next;
-      if (ql + 1 < nq_cta) issue(ql + 1);
+      if (ql + C::NG < nq_cta) issue(ql + C::NG);
       cp_async_commit();
-      if (pt < EG) si[pt] = meta_cur;
-      else if (pt >= 32 && pt < 32 + EG * Nfaces) si[EG + pt - 32] = meta_cur;
-      cp_async_wait_group<1>();   // everything of quad ql has landed (quad ql+1 may still be in flight)
-      producer_sync(PT);
+      if (pt < EG + EG * Nfaces) si[pt] = meta_cur;
+      cp_async_wait_group<1>();   // everything of quad ql has landed (the group's next quad may still be in flight)
+      producer_sync<PT>(grp);
       // ---- a5: upwind flux at my face nodes (eq. 7; reading R7), in place over the gathered q+
 #pragma unroll
       for (int r = 0; r < ((ALEGB_DBG & 1) ? 0 : ROUNDS); ++r) {
