@@ -49,13 +49,14 @@ struct Cfg {
   static constexpr int S = stride_pad(4 * KS);     // node stride of a q-tile row
   static constexpr int SG = stride_pad(4 * KFT);   // face-node stride of a flux-tile row
   static constexpr int EG = 4;                 // elements per quad
-  static constexpr int PW = 4;                 // producer warps
-  static constexpr int CW = 8;                 // consumer warps (12 warps = 3 per SM sub-partition -> 168 registers)
+  // warps: 3-D 4 + 8 (3 per SM sub-partition -> up to 168 registers); 2-D 6 + 10 (< 128 registers, so 4 per sub-partition fit)
+  static constexpr int PW = DIM == 2 ? 6 : 4;  // producer warps
+  static constexpr int CW = DIM == 2 ? 10 : 8; // consumer warps
   // Producer groups.  3-D: the four producer warps work on ONE quad together (a quad is 1400 doubles of q and 240
   // flux tasks at N=4) and the ring has 4 slots (a 5th costs more in L1 capacity than it gains).  2-D: a quad is a
   // few hundred doubles and 36 DMMA per item, the per-quad latency chain of the producers (indices -> copies ->
   // barrier -> flux) is what bounds the kernel (profiles/r1_v12_cfg3_stage_kernel.md), so every producer warp
-  // streams quads of its own (warp w takes quads w, w+4, ...) into a deeper ring.
+  // streams quads of its own (warp w takes quads w, w+6, ...) into a 16-slot ring.
 #ifdef ALEGB_PG
   static constexpr int PG = ALEGB_PG;
 #else
@@ -64,9 +65,10 @@ struct Cfg {
 #ifdef ALEGB_NS
   static constexpr int NS = ALEGB_NS;
 #else
-  static constexpr int NS = PG == 32 ? 12 : 4;         // slots in the ring
+  static constexpr int NS = PG == 32 ? 16 : 4;         // slots in the ring
 #endif
   static constexpr int NG = PW * 32 / PG;      // producer groups
+  static constexpr int TAG0 = PG >= 64 ? 32 : EG;   // first thread of a group that fetches boundary tags
   static constexpr int Threads = (PW + CW) * 32;
   static constexpr int PT = PG;                // threads producing one quad
   static constexpr int NTASK = EG * NFN;       // flux tasks per quad
@@ -126,6 +128,7 @@ __device__ __forceinline__ void prefetch_l2(const void* p, uint32_t bytes) {
 template <int NTHREADS>
 __device__ __forceinline__ void producer_sync(int group) {   // the threads of one producer group
   if constexpr (NTHREADS == 32) __syncwarp();
+  else if (group == 0) asm volatile("bar.sync 1, %0;" ::"n"(NTHREADS) : "memory");
   else asm volatile("bar.sync %0, %1;" ::"r"(1 + group), "n"(NTHREADS) : "memory");
 }
 
@@ -175,7 +178,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
     // Every global read of a quad is asynchronous (cp.async straight into its slot) and issued one quad ahead of
     // the flux arithmetic, so the producers never sit on a load: a group's iteration issues its next quad, then
     // computes the current one.
-    const int pt = tid % PT, grp = tid / PT;   // thread within its producer group, group
+    const int pt = C::NG == 1 ? tid : tid % PT, grp = C::NG == 1 ? 0 : tid / PT;   // thread within its producer group, group
     constexpr int ROUNDS = C::ROUNDS;
     int task_fe[ROUNDS], task_m[ROUNDS];
 #pragma unroll
@@ -185,7 +188,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       task_m[r] = task - task_fe[r] * NFN;
     }
     int idx_next[ROUNDS];   // vmapP entries of my face nodes in the quad that is issued next
-    int meta_next = 0;      // pml index (threads < EG) / boundary tag (threads EG .. EG+EG*Nfaces) of that quad
+    int meta_next = 0;      // pml index (threads < EG) / boundary tag (threads TAG0 .. TAG0+EG*Nfaces) of that quad
 
     auto load_indices = [&](int ql) {
       const int64_t e0 = ((int64_t)ql * gridDim.x + blockIdx.x) * EG;
@@ -230,8 +233,8 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       meta_next = pt < EG ? -1 : 0;
       if (pt < EG) {
         if (pt < nel && a.pml_index != nullptr && a.aux != nullptr) meta_next = __ldg(a.pml_index + e0 + pt);
-      } else if (pt < EG + EG * Nfaces) {
-        const int ef = pt - EG;
+      } else if (pt >= C::TAG0 && pt < C::TAG0 + EG * Nfaces) {
+        const int ef = pt - C::TAG0;
         if (ef < nel * Nfaces && a.EToB != nullptr) meta_next = a.EToB[e0 * Nfaces + ef];
       }
       // L2 prefetch of the a6 inputs the consumers will read for this quad
@@ -260,7 +263,8 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       const int meta_cur = meta_next;
       if (ql + C::NG < nq_cta) issue(ql + C::NG);
       cp_async_commit();
-      if (pt < EG + EG * Nfaces) si[pt] = meta_cur;
+      if (pt < EG) si[pt] = meta_cur;
+      else if (pt >= C::TAG0 && pt < C::TAG0 + EG * Nfaces) si[EG + pt - C::TAG0] = meta_cur;
       cp_async_wait_group<1>();   // everything of quad ql has landed (the group's next quad may still be in flight)
       producer_sync<PT>(grp);
       // ---- a5: upwind flux at my face nodes (eq. 7; reading R7), in place over the gathered q+
