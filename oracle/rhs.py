@@ -56,13 +56,17 @@ class Problem:
             self.pml_elems = np.zeros(0, dtype=np.int64)
 
     # -- a1 + a2: vertices and geometric factors at time t
-    def geometry(self, t):
-        xv, vv = _motion.vertices(self.motion_kind, self.motion_params, self.X0, t)
+    def geometry(self, t, verts=None):
+        """verts = (xv, vv) overrides the closed-form law (coordinates integrated in time, oracle/coords.py)."""
+        if verts is None:
+            xv, vv = _motion.vertices(self.motion_kind, self.motion_params, self.X0, t)
+        else:
+            xv, vv = verts
         g = _geometry.factors(self.dim, xv, self.EToV)
         g["xv"], g["vv"] = xv, vv
         return g
 
-    def rhs(self, q, t, aux=None, want_abs=False):
+    def rhs(self, q, t, aux=None, want_abs=False, verts=None):
         """q[K, Nf, Np] -> F[K, Nf, Np]   (and Faux[Kpml, dim, Nf, Np] if the mesh has a PML; and Fabs if asked).
 
         Fabs is the same sum with every term replaced by a bound on its absolute value: the scale against which a
@@ -70,7 +74,7 @@ class Problem:
         """
         ref, dim, c, K, Nf = self.ref, self.dim, self.c, self.K, self.Nf
         Np, Nfp, Nfaces = ref.Np, ref.Nfp, ref.Nfaces
-        g = self.geometry(t)
+        g = self.geometry(t, verts)
         Ginv = g["Ginv"]                                        # [K, a, d] = d xi_a / d x_d
         vG = np.einsum("iv,kvd->kid", ref.lam, g["vv"][self.EToV])   # [K, Np, dim]   (L152, L192)
 

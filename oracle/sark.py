@@ -48,8 +48,11 @@ def coefficients(gamma):
     return [[float(v) for v in row] for row in a], [float(v) for v in b]
 
 
-def step_debug(problem, q, t0, dt, aux=None):
-    """One SARK4 step.  Returns (stages, aux_new): stages = [q^(1), q^(2), q^(3), q_{n+1}] (L132-134)."""
+def step_debug(problem, q, t0, dt, aux=None, verts=None):
+    """One SARK4 step.  Returns (stages, aux_new): stages = [q^(1), q^(2), q^(3), q_{n+1}] (L132-134).
+
+    verts: optional list of four (xv, vv) pairs, the vertex positions / velocities of the four stages when the
+    coordinates are integrated in time (oracle/coords.py) instead of evaluated from the closed-form law."""
     dim = problem.dim
     stiff = _physics.stiff_mask(dim)                         # 1 where Lambda = 1/tau
     lam = stiff / problem.tau
@@ -68,11 +71,12 @@ def step_debug(problem, q, t0, dt, aux=None):
     qi, auxi = q, aux
     for i in range(4):
         ti = t0 + RK4_C[i] * dt
+        vi = None if verts is None else verts[i]
         if has_pml:
-            Fi, Gi = problem.rhs(qi, ti, aux=auxi)
+            Fi, Gi = problem.rhs(qi, ti, aux=auxi, verts=vi)
             Gs.append(Gi)
         else:
-            Fi = problem.rhs(qi, ti)
+            Fi = problem.rhs(qi, ti, verts=vi)
         Fs.append(Fi)
         if i < 3:
             ci = RK4_C[i + 1]
