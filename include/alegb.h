@@ -74,6 +74,15 @@ typedef enum {
   ALEGB_MOTION_USER = 5
 } alegb_motion_kind;
 
+/* How alegb_step / alegb_step_debug obtain the vertex positions of a stage.
+ *   CLOSED_FORM  x_v(t_i) = X0_v + disp(X0_v, t_i) from the law (reading R9; default)
+ *   RK           the coordinates are "advanced in time using the same Runge-Kutta integration scheme employed for the
+ *                primary solver" (L152; L233 dx/dt = v_G): classic RK4 on dx/dt = v(X0, t) with the law's vertex
+ *                velocity; stage i sees x^(i) = x_n + dt a_{i,i-1} v(t_{i-1}) and the velocity v(t_i), and the step
+ *                ends with x_{n+1} = x_n + dt sum_j b_j v(t_j).  Motion kind USER: the supplied velocity, constant in
+ *                time.  (SURVEY 8(f) NEXT-2.)  alegb_rhs and alegb_geometry always evaluate the closed form. */
+typedef enum { ALEGB_COORDS_CLOSED_FORM = 0, ALEGB_COORDS_RK = 1 } alegb_coord_mode;
+
 /* Create a context for simplices of dimension dim (2 or 3) and polynomial order N (1..ALEGB_MAX_N) on CUDA device
  * `cuda_device`.  Builds the reference element on the host: Warp & Blend nodes (L75), D_r,D_s(,D_t) = M^-1 S and
  * LIFT = M^-1 M^f (L94-103).  *out is NULL on failure. */
@@ -101,6 +110,15 @@ int alegb_set_motion(alegb_ctx* ctx, int kind, const double* params, int nparams
 /* kind USER: DEVICE arrays [Nverts*dim] of vertex positions and velocities, copied device-to-device on the
  * default stream and used for every subsequent evaluation until the motion is set again. */
 int alegb_set_motion_user(alegb_ctx* ctx, const double* d_xv, const double* d_vv);
+
+/* Select the coordinate mode.  RK: the library's current positions x_n are set to the law's positions at t_start
+ * (kind USER: to the positions last given to alegb_set_motion_user); every alegb_step then advances them, so
+ * consecutive calls must continue in time where the previous one ended.  alegb_step_debug reads x_n and leaves it
+ * unchanged.  Synchronises.  Errors: INVALID_ARG (mode), NOT_READY (no mesh), CUDA_ERROR. */
+int alegb_set_coordinate_mode(alegb_ctx* ctx, int mode, double t_start);
+/* Current vertex positions, DEVICE out [Nverts*dim]: x_n in RK mode, else the positions of the last evaluation.
+ * Enqueued on `stream`, does not synchronise. */
+int alegb_get_positions(alegb_ctx* ctx, double* d_x, void* stream);
 
 /* F = L(q) + N~(q) at time t (no -Lambda q), DEVICE q, F [K][Nf][Np].  In PML elements the library's current
  * auxiliary fields enter F (term - sum_d sigma_d q~^d). */

@@ -14,6 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libalegb.so")
 
 OK, INVALID_ARG, BAD_MESH, NOT_READY, UNSUPPORTED, CUDA_ERROR = 0, -1, -2, -3, -4, -5
 MOTION_NONE, MOTION_SINES_PRODUCT, MOTION_SINES_CROSS, MOTION_PLUNGE_BLEND, MOTION_CARANGIFORM, MOTION_USER = range(6)
+COORDS_CLOSED_FORM, COORDS_RK = 0, 1
 STATUS_NAMES = {0: "OK", -1: "INVALID_ARG", -2: "BAD_MESH", -3: "NOT_READY", -4: "UNSUPPORTED", -5: "CUDA_ERROR"}
 
 if not os.path.exists(LIB_PATH):
@@ -30,6 +31,8 @@ _SIGNATURES = {
     "alegb_set_params": (_c.c_int, [_P, _c.c_double, _c.c_double, _P]),
     "alegb_set_motion": (_c.c_int, [_P, _c.c_int, _P, _c.c_int]),
     "alegb_set_motion_user": (_c.c_int, [_P, _P, _P]),
+    "alegb_set_coordinate_mode": (_c.c_int, [_P, _c.c_int, _c.c_double]),
+    "alegb_get_positions": (_c.c_int, [_P, _P, _P]),
     "alegb_rhs": (_c.c_int, [_P, _c.c_double, _P, _P, _P]),
     "alegb_rhs_pml": (_c.c_int, [_P, _c.c_double, _P, _P, _P, _P, _P]),
     "alegb_step": (_c.c_int, [_P, _P, _c.c_double, _c.c_double, _c.c_int, _P]),
@@ -139,6 +142,12 @@ class Context:
 
     def alegb_set_motion_user(self, d_xv, d_vv):
         self._check(_lib.alegb_set_motion_user(self._h, _dev(d_xv), _dev(d_vv)))
+
+    def alegb_set_coordinate_mode(self, mode, t_start=0.0):
+        self._check(_lib.alegb_set_coordinate_mode(self._h, int(mode), float(t_start)))
+
+    def alegb_get_positions(self, d_x, stream=None):
+        self._check(_lib.alegb_get_positions(self._h, _dev(d_x), _stream(stream)))
 
     # ---- compute (device arrays)
     def alegb_rhs(self, t, d_q, d_F, stream=None):

@@ -30,6 +30,9 @@ struct alegb_ctx {
   int kernel_mode = 0;   // 0 auto (pipelined DMMA, else DMMA, else generic), 1 generic, 2 pipelined DMMA, 3 warp-per-quad DMMA
   // device: mesh
   double *d_X0 = nullptr, *d_xv = nullptr, *d_vv = nullptr;
+  // NEXT-2: coordinates integrated by RK4: current positions x_n, the user's constant velocity
+  int coord_mode = ALEGB_COORDS_CLOSED_FORM;
+  double *d_xn = nullptr, *d_user_vv = nullptr;
   int32_t *d_EToV = nullptr, *d_vmapP = nullptr;
   int8_t* d_EToB = nullptr;
   double *d_vgeo = nullptr, *d_sgeo = nullptr, *d_vvel = nullptr;
@@ -90,6 +93,7 @@ void dev_free(T*& p) {
 }
 
 void free_mesh(alegb_ctx* ctx) {
+  dev_free(ctx->d_xn); dev_free(ctx->d_user_vv); ctx->coord_mode = ALEGB_COORDS_CLOSED_FORM;
   dev_free(ctx->d_X0); dev_free(ctx->d_xv); dev_free(ctx->d_vv); dev_free(ctx->d_EToV); dev_free(ctx->d_vmapP);
   dev_free(ctx->d_EToB); dev_free(ctx->d_vgeo); dev_free(ctx->d_sgeo); dev_free(ctx->d_vvel);
   dev_free(ctx->d_pml_index); dev_free(ctx->d_pml_elems); dev_free(ctx->d_pml_sigma);
@@ -111,6 +115,21 @@ int update_geometry(alegb_ctx* ctx, double t, cudaStream_t s, const double* t_de
   }
   CU(launch_geometry(dim, ctx->K, ctx->d_EToV, ctx->d_xv, ctx->d_vv, ctx->d_vgeo, ctx->d_sgeo, ctx->d_vvel, s));
   ctx->launches++;
+  return ALEGB_OK;
+}
+
+// a1 + a2 of stage `stage` of the step starting at t0 when the coordinates are integrated in time (NEXT-2);
+// stage 4 = end of the step (x_n <- x_{n+1}, no geometry)
+int update_geometry_rk(alegb_ctx* ctx, int stage, double t0, double dt, cudaStream_t s, const double* ts_dev) {
+  const int dim = ctx->ref.dim;
+  const double* uvv = ctx->motion.kind == ALEGB_MOTION_USER ? ctx->d_user_vv : nullptr;
+  CU(launch_vertex_rk(dim, ctx->Nverts, ctx->d_X0, ctx->motion, uvv, stage, t0, t0 + 0.5 * dt, t0 + 1.0 * dt, dt, ts_dev,
+                      ctx->d_xn, ctx->d_xv, ctx->d_vv, s));
+  ctx->launches++;
+  if (stage < 4) {
+    CU(launch_geometry(dim, ctx->K, ctx->d_EToV, ctx->d_xv, ctx->d_vv, ctx->d_vgeo, ctx->d_sgeo, ctx->d_vvel, s));
+    ctx->launches++;
+  }
   return ALEGB_OK;
 }
 
@@ -177,7 +196,7 @@ int timed_stage(alegb_ctx* ctx, const StageArgs& a, cudaStream_t s) {
 // One SARK4 step.  q_n: state at t0 (read only); outs[i]: where stage state i+1 is written
 // (outs[3] = q_{n+1}, may alias q_n).
 int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t0, double dt, cudaStream_t s,
-              const double* t_dev = nullptr) {
+              const double* t_dev = nullptr, bool advance_coords = true) {
   const int dim = ctx->ref.dim, N = ctx->ref.N, Nf = ctx->Nf;
   const double gamma = -dt * ctx->invtau;  // L144
   double as[6], bs[4], a0[6], b0[4];
@@ -197,7 +216,8 @@ int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t
   const bool pml = ctx->Kpml > 0;
   for (int i = 0; i < 4; ++i) {
     const double ti = t0 + cstage[i] * dt;
-    int rc = update_geometry(ctx, ti, s, t_dev ? t_dev + i : nullptr);
+    int rc = ctx->coord_mode == ALEGB_COORDS_RK ? update_geometry_rk(ctx, i, t0, dt, s, t_dev)
+                                                 : update_geometry(ctx, ti, s, t_dev ? t_dev + i : nullptr);
     if (rc != ALEGB_OK) return rc;
     StageArgs a;
     fill_common(ctx, a);
@@ -246,6 +266,7 @@ int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t
       ctx->launches++;
     }
   }
+  if (ctx->coord_mode == ALEGB_COORDS_RK && advance_coords) return update_geometry_rk(ctx, 4, t0, dt, s, t_dev);
   return ALEGB_OK;
 }
 
@@ -526,9 +547,43 @@ int alegb_set_motion_user(alegb_ctx* ctx, const double* d_xv, const double* d_vv
   const size_t bytes = (size_t)ctx->Nverts * ctx->ref.dim * sizeof(double);
   CU(cudaMemcpyAsync(ctx->d_xv, d_xv, bytes, cudaMemcpyDeviceToDevice, 0));
   CU(cudaMemcpyAsync(ctx->d_vv, d_vv, bytes, cudaMemcpyDeviceToDevice, 0));
+  if (!ctx->d_user_vv) CU(dev_alloc(ctx, &ctx->d_user_vv, (size_t)ctx->Nverts * ctx->ref.dim));
+  CU(cudaMemcpyAsync(ctx->d_user_vv, d_vv, bytes, cudaMemcpyDeviceToDevice, 0));
   CU(cudaStreamSynchronize(0));
   ctx->motion.kind = ALEGB_MOTION_USER;
   ctx->config_version++;
+  return ALEGB_OK;
+}
+
+int alegb_set_coordinate_mode(alegb_ctx* ctx, int mode, double t_start) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  if (mode != ALEGB_COORDS_CLOSED_FORM && mode != ALEGB_COORDS_RK) return fail(ctx, ALEGB_INVALID_ARG, "unknown coordinate mode");
+  if (mode == ALEGB_COORDS_RK) {
+    if (ctx->device < 0) return fail(ctx, ALEGB_CUDA_ERROR, "host-only context (no CUDA device)");
+    if (!ctx->mesh_ready) return fail(ctx, ALEGB_NOT_READY, "alegb_mesh_upload has not been called");
+    CU(cudaSetDevice(ctx->device));
+    const int dim = ctx->ref.dim;
+    if (!ctx->d_xn) CU(dev_alloc(ctx, &ctx->d_xn, (size_t)ctx->Nverts * dim));
+    // x_n = the law's own position at t_start (USER: the positions last supplied)
+    if (ctx->motion.kind != ALEGB_MOTION_USER)
+      CU(launch_vertex_motion(dim, ctx->Nverts, ctx->d_X0, ctx->motion, t_start, nullptr, ctx->d_xv, ctx->d_vv, 0));
+    CU(cudaMemcpyAsync(ctx->d_xn, ctx->d_xv, (size_t)ctx->Nverts * dim * sizeof(double), cudaMemcpyDeviceToDevice, 0));
+    CU(cudaStreamSynchronize(0));
+  }
+  ctx->coord_mode = mode;
+  ctx->config_version++;
+  return ALEGB_OK;
+}
+
+int alegb_get_positions(alegb_ctx* ctx, double* d_x, void* stream) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  if (ctx->device < 0) return fail(ctx, ALEGB_CUDA_ERROR, "host-only context (no CUDA device)");
+  if (!ctx->mesh_ready) return fail(ctx, ALEGB_NOT_READY, "alegb_mesh_upload has not been called");
+  if (!d_x) return fail(ctx, ALEGB_INVALID_ARG, "NULL device array");
+  CU(cudaSetDevice(ctx->device));
+  const double* src = ctx->coord_mode == ALEGB_COORDS_RK ? ctx->d_xn : ctx->d_xv;
+  CU(cudaMemcpyAsync(d_x, src, (size_t)ctx->Nverts * ctx->ref.dim * sizeof(double), cudaMemcpyDeviceToDevice,
+                     static_cast<cudaStream_t>(stream)));
   return ALEGB_OK;
 }
 
@@ -586,7 +641,7 @@ int alegb_step_debug(alegb_ctx* ctx, const double* d_q, double t0, double dt, do
   if (!aligned16(d_q) || !aligned16(d_stages)) return fail(ctx, ALEGB_INVALID_ARG, "field pointers must be 16-byte aligned");
   const size_t state = (size_t)ctx->K * ctx->Nf * ctx->ref.Np;
   double* outs[4] = {d_stages, d_stages + state, d_stages + 2 * state, d_stages + 3 * state};
-  return sark_step(ctx, d_q, outs, t0, dt, (cudaStream_t)stream);
+  return sark_step(ctx, d_q, outs, t0, dt, (cudaStream_t)stream, nullptr, /*advance_coords=*/false);
 }
 
 int alegb_step_host(alegb_ctx* ctx, double* h_q, double t0, double dt, int nsteps) {

@@ -86,6 +86,10 @@ struct MotionArgs {
 // t_dev != NULL: the stage time is read from the device (graph-captured steps) and t is ignored
 cudaError_t launch_vertex_motion(int dim, int64_t Nverts, const double* X0, const MotionArgs& m, double t,
                                  const double* t_dev, double* xv, double* vv, cudaStream_t s);
+// coordinates integrated by RK4 (NEXT-2): stage 0..3 writes xv, vv of that stage; stage 4 advances x_n to x_{n+1}
+cudaError_t launch_vertex_rk(int dim, int64_t Nverts, const double* X0, const MotionArgs& m, const double* user_vv,
+                             int stage, double t_n, double t_h, double t_e, double dt, const double* ts_dev, double* x_n,
+                             double* xv, double* vv, cudaStream_t s);
 // clock = {t0, dt, stage times[4]} on the device; _set starts a run of steps, the other advances to the next step
 cudaError_t launch_step_clock(double* clock, long long* counter, cudaStream_t s);
 cudaError_t launch_step_clock_set(double* clock, long long* counter, double t0, double dt, cudaStream_t s);

@@ -14,17 +14,12 @@
 namespace alegb {
 
 // ------------------------------------------------------------------------------------------------------------------
-// a1: vertex motion.  One thread per vertex.
+// The prescribed motion laws at one vertex: displacement and velocity at time t from the t = 0 coordinate X
+// (include/alegb.h lists the parameters).
 template <int DIM>
-__global__ void vertex_motion_kernel(int64_t Nverts, const double* __restrict__ X0, MotionArgs m, double t,
-                                     const double* __restrict__ t_dev, double* __restrict__ xv,
-                                     double* __restrict__ vv) {
-  int64_t v = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-  if (v >= Nverts) return;
-  if (t_dev != nullptr) t = *t_dev;   // stage time kept on the device (graph-captured steps)
-  double X[DIM], disp[DIM], vel[DIM];
+__device__ __forceinline__ void motion_law(const MotionArgs& m, const double* X, double t, double* disp, double* vel) {
 #pragma unroll
-  for (int d = 0; d < DIM; ++d) { X[d] = X0[v * DIM + d]; disp[d] = 0.0; vel[d] = 0.0; }
+  for (int d = 0; d < DIM; ++d) { disp[d] = 0.0; vel[d] = 0.0; }
   const double* p = m.p;
   if (m.kind == 1) {  // SINES_PRODUCT: eq. 15
     double A = p[0], om = 2.0 * M_PI / p[1], shape = 1.0;
@@ -80,8 +75,75 @@ __global__ void vertex_motion_kernel(int64_t Nverts, const double* __restrict__ 
         vel[d] = -Amp * om * cos(phi) * B * S + Amp * sin(phi) * B * Sd;
       }
   }
+}
+
+// a1: vertex motion.  One thread per vertex.
+template <int DIM>
+__global__ void vertex_motion_kernel(int64_t Nverts, const double* __restrict__ X0, MotionArgs m, double t,
+                                     const double* __restrict__ t_dev, double* __restrict__ xv,
+                                     double* __restrict__ vv) {
+  int64_t v = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (v >= Nverts) return;
+  if (t_dev != nullptr) t = *t_dev;   // stage time kept on the device (graph-captured steps)
+  double X[DIM], disp[DIM], vel[DIM];
+#pragma unroll
+  for (int d = 0; d < DIM; ++d) X[d] = X0[v * DIM + d];
+  motion_law<DIM>(m, X, t, disp, vel);
 #pragma unroll
   for (int d = 0; d < DIM; ++d) { xv[v * DIM + d] = X[d] + disp[d]; vv[v * DIM + d] = vel[d]; }
+}
+
+// a1, coordinates integrated in time ("the nodal coordinates are advanced in time using the same
+// Runge-Kutta integration scheme", L233 dx/dt = v_G).  Classic RK4 on dx/dt = v(X0, t):
+//   stage 0: x_n, v(t_n)   1: x_n + dt/2 v(t_n), v(t_h)   2: x_n + dt/2 v(t_h), v(t_h)   3: x_n + dt v(t_h), v(t_n+dt)
+//   stage 4 (end of the step): x_n <- x_n + dt/6 (v(t_n) + 2 v(t_h) + 2 v(t_h) + v(t_n+dt))
+// The velocities are re-evaluated from the law (a few sincos per vertex) instead of being kept between launches;
+// user_vv != NULL: a velocity that is constant in time (motion kind USER).
+// ts = {t_n, t_h, t_h, t_n + dt}; ts_dev (graph-captured steps) points at the same four times on the device, with dt
+// one double before them (the step clock).
+template <int DIM>
+__global__ void vertex_rk_kernel(int64_t Nverts, const double* __restrict__ X0, MotionArgs m,
+                                 const double* __restrict__ user_vv, int stage, double t_n, double t_h, double t_e,
+                                 double dt, const double* __restrict__ ts_dev, double* __restrict__ x_n,
+                                 double* __restrict__ xv, double* __restrict__ vv) {
+  int64_t v = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (v >= Nverts) return;
+  if (ts_dev != nullptr) { t_n = ts_dev[0]; t_h = ts_dev[1]; t_e = ts_dev[3]; dt = ts_dev[-1]; }
+  double X[DIM], xn[DIM], disp[DIM], k1[DIM], k2[DIM], k4[DIM];
+#pragma unroll
+  for (int d = 0; d < DIM; ++d) { X[d] = X0[v * DIM + d]; xn[d] = x_n[v * DIM + d]; }
+  if (user_vv != nullptr) {
+#pragma unroll
+    for (int d = 0; d < DIM; ++d) k1[d] = k2[d] = k4[d] = user_vv[v * DIM + d];
+  } else {
+    motion_law<DIM>(m, X, t_n, disp, k1);
+    motion_law<DIM>(m, X, t_h, disp, k2);
+    motion_law<DIM>(m, X, t_e, disp, k4);
+  }
+#pragma unroll
+  for (int d = 0; d < DIM; ++d) {
+    double x, w;
+    if (stage == 0) { x = xn[d]; w = k1[d]; }
+    else if (stage == 1) { x = fma(0.5 * dt, k1[d], xn[d]); w = k2[d]; }
+    else if (stage == 2) { x = fma(0.5 * dt, k2[d], xn[d]); w = k2[d]; }
+    else if (stage == 3) { x = fma(dt, k2[d], xn[d]); w = k4[d]; }
+    else {
+      x_n[v * DIM + d] = xn[d] + dt * ((1.0 / 6.0) * k1[d] + (1.0 / 3.0) * k2[d] + (1.0 / 3.0) * k2[d] + (1.0 / 6.0) * k4[d]);
+      continue;
+    }
+    xv[v * DIM + d] = x;
+    vv[v * DIM + d] = w;
+  }
+}
+
+cudaError_t launch_vertex_rk(int dim, int64_t Nverts, const double* X0, const MotionArgs& m, const double* user_vv,
+                             int stage, double t_n, double t_h, double t_e, double dt, const double* ts_dev, double* x_n,
+                             double* xv, double* vv, cudaStream_t s) {
+  if (Nverts == 0) return cudaSuccess;
+  int nb = (int)((Nverts + 255) / 256);
+  if (dim == 2) vertex_rk_kernel<2><<<nb, 256, 0, s>>>(Nverts, X0, m, user_vv, stage, t_n, t_h, t_e, dt, ts_dev, x_n, xv, vv);
+  else vertex_rk_kernel<3><<<nb, 256, 0, s>>>(Nverts, X0, m, user_vv, stage, t_n, t_h, t_e, dt, ts_dev, x_n, xv, vv);
+  return cudaGetLastError();
 }
 
 cudaError_t launch_vertex_motion(int dim, int64_t Nverts, const double* X0, const MotionArgs& m, double t,

@@ -414,3 +414,85 @@ def test_full_size_throughput_config_sampled(refs, B):
     torch.cuda.synchronize()
     assert np.abs(dq.cpu().numpy() - q0).max() < 1e-13
     ctx.close()
+
+
+# ------------------------------------------------------------------ NEXT-2: coordinates integrated by RK4 (L152, L233)
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", ["cfg1", "cfg3", "cfg4"])
+def test_rk_coordinates_stage_states_match_oracle(name, refs, B):
+    """alegb_set_coordinate_mode(RK): stage states of one step from an advanced x_n, positions after several steps."""
+    from oracle import coords
+    ref, cfg = make_case(name, refs)
+    P = oracle_problem(cfg, ref)
+    q = perturbed(cfg)
+    dt, t0 = cfg["dt"], 0.0
+    ctx = B.context_from_config(cfg)
+    ctx.alegb_set_coordinate_mode(B.COORDS_RK, t0)
+    # two steps through alegb_step advance q and x_n; the oracle does the same
+    dq = dev(q)
+    ctx.alegb_step(dq, t0, dt, 2)
+    dx = torch.empty(cfg["X0"].shape, dtype=torch.float64, device="cuda")
+    ctx.alegb_get_positions(dx)
+    torch.cuda.synchronize()
+    if P.sigma is not None:
+        qo, xo, auxo = coords.step(P, q, P.X0.copy(), t0, dt, 2)
+    else:
+        qo, xo = coords.step(P, q, P.X0.copy(), t0, dt, 2)
+        auxo = None
+    assert np.abs(dx.cpu().numpy() - xo).max() <= 1e-14 * max(1.0, np.abs(xo).max())
+    assert rel_linf(dq.cpu().numpy(), qo) <= 2 * TOL_STAGE
+    # the third step observed stage by stage; step_debug must leave x_n alone
+    st = torch.empty((4,) + q.shape, dtype=torch.float64, device="cuda")
+    ctx.alegb_step_debug(dq, t0 + 2 * dt, dt, st)
+    dx2 = torch.empty_like(dx)
+    ctx.alegb_get_positions(dx2)
+    torch.cuda.synchronize()
+    assert torch.equal(dx, dx2)
+    so, _, _ = coords.step_debug(P, qo, xo, t0 + 2 * dt, dt, auxo)
+    for i in range(4):
+        assert rel_linf(st[i].cpu().numpy(), so[i]) <= 2 * TOL_STAGE
+    ctx.close()
+
+
+@pytest.mark.gpu
+def test_rk_coordinates_graph_replay_and_free_stream(refs, B):
+    """Many steps through the captured graph equal the direct launches bit for bit, x_n included; a uniform state on
+    the integrated mesh stays uniform (GCL, Table 2)."""
+    ref, cfg = make_case("cfg1", refs)
+    q0 = cfg["q0"]
+    outs = []
+    for graph in (1, 0):
+        ctx = B.context_from_config(cfg)
+        ctx.alegb_set_graph(graph)
+        ctx.alegb_set_coordinate_mode(B.COORDS_RK, 0.0)
+        dq = dev(q0)
+        ctx.alegb_step(dq, 0.0, cfg["dt"], 25)
+        dx = torch.empty(cfg["X0"].shape, dtype=torch.float64, device="cuda")
+        ctx.alegb_get_positions(dx)
+        torch.cuda.synchronize()
+        outs.append((dq.cpu().numpy(), dx.cpu().numpy()))
+        ctx.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    assert np.abs(outs[0][0] - q0).max() < 1e-13
+    exact = omotion.vertices(cfg["motion_kind"], cfg["motion_params"], cfg["X0"], 25 * cfg["dt"])[0]
+    assert np.abs(outs[0][1] - exact).max() < 1e-8             # follows the law to time-integration accuracy
+
+
+@pytest.mark.gpu
+def test_rk_coordinates_user_velocity(refs, B):
+    """Motion kind USER in RK mode: a velocity constant in time moves the vertices linearly."""
+    ref, cfg = make_case("cfg1", refs)
+    rng = np.random.default_rng(199)
+    xv = cfg["X0"].copy()
+    vv = 0.05 * np.sin(np.pi * cfg["X0"][:, :1]) * np.sin(np.pi * cfg["X0"][:, 1:2]) * np.ones((1, 2))
+    ctx = B.context_from_config(cfg)
+    ctx.alegb_set_motion_user(dev(xv), dev(vv))
+    ctx.alegb_set_coordinate_mode(B.COORDS_RK, 0.0)
+    dq = dev(cfg["q0"])
+    ctx.alegb_step(dq, 0.0, cfg["dt"], 10)
+    dx = torch.empty(xv.shape, dtype=torch.float64, device="cuda")
+    ctx.alegb_get_positions(dx)
+    torch.cuda.synchronize()
+    assert np.abs(dx.cpu().numpy() - (xv + 10 * cfg["dt"] * vv)).max() < 1e-15
+    assert np.abs(dq.cpu().numpy() - cfg["q0"]).max() < 1e-13       # free stream
+    ctx.close()
