@@ -25,6 +25,7 @@ from . import geometry as _geometry
 from . import mesh as _mesh
 from . import motion as _motion
 from . import physics as _physics
+from . import cubature as _cubature
 from .operators import ReferenceElement
 
 WALL, FARFIELD = 1, 2
@@ -34,7 +35,7 @@ class Problem:
     """Everything F(q, t) needs besides q and t.  Mirrors the arguments of the C-ABI (mesh upload, params, motion)."""
 
     def __init__(self, dim, N, X0, EToV, vertex_equiv=None, EToB=None, pml_sigma=None,
-                 RT=1.0, tau=1.0, q_inf=None, motion_kind=0, motion_params=None, ref=None):
+                 RT=1.0, tau=1.0, q_inf=None, motion_kind=0, motion_params=None, ref=None, relax="collocation"):
         self.dim, self.N = dim, N
         self.ref = ref if ref is not None else ReferenceElement(dim, N)
         self.X0 = np.ascontiguousarray(X0, dtype=float)
@@ -47,6 +48,11 @@ class Problem:
         self.q_inf = None if q_inf is None else np.asarray(q_inf, dtype=float)
         self.motion_kind, self.motion_params = motion_kind, motion_params
         self.Nf = _physics.nfields(dim)
+        # nonlinear relaxation: collocated at the interpolation nodes (reading R8) or cubature-projected (L84-107, L197)
+        if relax not in ("collocation", "cubature"):
+            raise ValueError("relax must be 'collocation' or 'cubature'")
+        self.relax = relax
+        self.cub = _cubature.Cubature(self.ref) if relax == "cubature" else None
         self.A = _physics.stream_matrices(dim)
         if pml_sigma is not None and np.any(np.asarray(pml_sigma) > 0):
             self.sigma = np.asarray(pml_sigma, dtype=float).reshape(self.K, dim)
@@ -92,12 +98,18 @@ class Problem:
             sd = -c * np.einsum("fg,kgi->kfi", self.A[d], grad[d])
             stream_d.append(sd)
             F += sd + vG[:, None, :, d] * grad[d]
-        # ---- collocated relaxation (L115; reading R8)
-        F += _physics.N_tilde(dim, q, self.tau)
+        # ---- nonlinear relaxation N~ (L115): collocated (reading R8) or P N~(I q) (eq. 9 last term, L197)
+        if self.cub is None:
+            F += _physics.N_tilde(dim, q, self.tau)
+        else:
+            F += _cubature.relaxation(self.cub, dim, q, self.tau)
 
         if want_abs:
             aref = [np.einsum("ij,kfj->kfi", np.abs(ref.D[a]), np.abs(q)) for a in range(dim)]
-            Fabs = np.abs(_physics.N_tilde(dim, q, self.tau))
+            if self.cub is None:
+                Fabs = np.abs(_physics.N_tilde(dim, q, self.tau))
+            else:
+                Fabs = _cubature.relaxation_abs(self.cub, dim, q, self.tau)
             for d in range(dim):
                 gabs = 0.0
                 for a in range(dim):

@@ -6,7 +6,8 @@ def oracle_problem(cfg, ref):
     from oracle.rhs import Problem
     return Problem(cfg["dim"], cfg["N"], cfg["X0"], cfg["EToV"], cfg.get("vertex_equiv"), cfg.get("EToB"),
                    cfg.get("pml_sigma"), RT=cfg["RT"], tau=cfg["tau"], q_inf=cfg.get("q_inf"),
-                   motion_kind=cfg["motion_kind"], motion_params=cfg["motion_params"], ref=ref)
+                   motion_kind=cfg["motion_kind"], motion_params=cfg["motion_params"], ref=ref,
+                   relax=cfg.get("relax", "collocation"))
 
 
 def rel_linf(a, b):
