@@ -83,6 +83,13 @@ typedef enum {
  *                time.  (SURVEY 8(f) NEXT-2.)  alegb_rhs and alegb_geometry always evaluate the closed form. */
 typedef enum { ALEGB_COORDS_CLOSED_FORM = 0, ALEGB_COORDS_RK = 1 } alegb_coord_mode;
 
+/* How the nonlinear relaxation N~(q) enters F.
+ *   COLLOCATION  evaluated at the interpolation nodes (reading R8; default)
+ *   CUBATURE     P N~(I q) of eq. 9 (L84-107; cubature kernel, L197): q interpolated to the N_c nodes of a
+ *                conical-product Gauss-Jacobi rule exact to degree 3N, N~ evaluated there, projected back with
+ *                P = M^-1 I^T diag(w).  (the rule is this build's choice, reading R20.) */
+typedef enum { ALEGB_RELAX_COLLOCATION = 0, ALEGB_RELAX_CUBATURE = 1 } alegb_relax_mode;
+
 /* Create a context for simplices of dimension dim (2 or 3) and polynomial order N (1..ALEGB_MAX_N) on CUDA device
  * `cuda_device`.  Builds the reference element on the host: Warp & Blend nodes (L75), D_r,D_s(,D_t) = M^-1 S and
  * LIFT = M^-1 M^f (L94-103).  *out is NULL on failure. */
@@ -110,6 +117,14 @@ int alegb_set_motion(alegb_ctx* ctx, int kind, const double* params, int nparams
 /* kind USER: DEVICE arrays [Nverts*dim] of vertex positions and velocities, copied device-to-device on the
  * default stream and used for every subsequent evaluation until the motion is set again. */
 int alegb_set_motion_user(alegb_ctx* ctx, const double* d_xv, const double* d_vv);
+
+/* Select the relaxation mode for alegb_rhs / alegb_step (every stage kernel honours it).  CUBATURE builds the rule
+ * and I, P on the host, uploads them and allocates R[K][dim(dim+1)/2][Np] (part of alegb_workspace_bytes).
+ * Synchronises.  Errors: INVALID_ARG, NOT_READY (no mesh), CUDA_ERROR. */
+int alegb_set_relaxation(alegb_ctx* ctx, int mode);
+/* The cubature rule and operators, HOST out, any pointer may be NULL: degree, Nc, rst[dim][Nc], w[Nc],
+ * I[Nc][Np] (L86), P[Np][Nc] (L103).  Call with the arrays NULL first to learn Nc.  Works on host-only contexts. */
+int alegb_get_cubature(alegb_ctx* ctx, int* degree, int* Nc, double* rst, double* w, double* I, double* P);
 
 /* Select the coordinate mode.  RK: the library's current positions x_n are set to the law's positions at t_start
  * (kind USER: to the positions last given to alegb_set_motion_user); every alegb_step then advances them, so

@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libalegb.so")
 OK, INVALID_ARG, BAD_MESH, NOT_READY, UNSUPPORTED, CUDA_ERROR = 0, -1, -2, -3, -4, -5
 MOTION_NONE, MOTION_SINES_PRODUCT, MOTION_SINES_CROSS, MOTION_PLUNGE_BLEND, MOTION_CARANGIFORM, MOTION_USER = range(6)
 COORDS_CLOSED_FORM, COORDS_RK = 0, 1
+RELAX_COLLOCATION, RELAX_CUBATURE = 0, 1
 STATUS_NAMES = {0: "OK", -1: "INVALID_ARG", -2: "BAD_MESH", -3: "NOT_READY", -4: "UNSUPPORTED", -5: "CUDA_ERROR"}
 
 if not os.path.exists(LIB_PATH):
@@ -32,6 +33,8 @@ _SIGNATURES = {
     "alegb_set_motion": (_c.c_int, [_P, _c.c_int, _P, _c.c_int]),
     "alegb_set_motion_user": (_c.c_int, [_P, _P, _P]),
     "alegb_set_coordinate_mode": (_c.c_int, [_P, _c.c_int, _c.c_double]),
+    "alegb_set_relaxation": (_c.c_int, [_P, _c.c_int]),
+    "alegb_get_cubature": (_c.c_int, [_P, _c.POINTER(_c.c_int), _c.POINTER(_c.c_int), _P, _P, _P, _P]),
     "alegb_get_positions": (_c.c_int, [_P, _P, _P]),
     "alegb_rhs": (_c.c_int, [_P, _c.c_double, _P, _P, _P]),
     "alegb_rhs_pml": (_c.c_int, [_P, _c.c_double, _P, _P, _P, _P, _P]),
@@ -142,6 +145,19 @@ class Context:
 
     def alegb_set_motion_user(self, d_xv, d_vv):
         self._check(_lib.alegb_set_motion_user(self._h, _dev(d_xv), _dev(d_vv)))
+
+    def alegb_set_relaxation(self, mode):
+        self._check(_lib.alegb_set_relaxation(self._h, int(mode)))
+
+    def alegb_get_cubature(self):
+        """-> dict(degree, Nc, rst[dim, Nc], w[Nc], I[Nc, Np], P[Np, Nc]) (host arrays)."""
+        deg, nc = _c.c_int(0), _c.c_int(0)
+        self._check(_lib.alegb_get_cubature(self._h, _c.byref(deg), _c.byref(nc), None, None, None, None))
+        dim, Np, Nc = self.dim, self.Np, nc.value
+        rst, w = np.empty((dim, Nc)), np.empty(Nc)
+        I, P = np.empty((Nc, Np)), np.empty((Np, Nc))
+        self._check(_lib.alegb_get_cubature(self._h, None, None, rst.ctypes.data, w.ctypes.data, I.ctypes.data, P.ctypes.data))
+        return dict(degree=deg.value, Nc=Nc, rst=rst, w=w, I=I, P=P)
 
     def alegb_set_coordinate_mode(self, mode, t_start=0.0):
         self._check(_lib.alegb_set_coordinate_mode(self._h, int(mode), float(t_start)))

@@ -32,6 +32,11 @@ struct alegb_ctx {
   double *d_X0 = nullptr, *d_xv = nullptr, *d_vv = nullptr;
   // NEXT-2: coordinates integrated by RK4: current positions x_n, the user's constant velocity
   int coord_mode = ALEGB_COORDS_CLOSED_FORM;
+  // NEXT-1: cubature-projected relaxation
+  int relax_mode = ALEGB_RELAX_COLLOCATION;
+  Cubature cub;                       // host copy (built on first use)
+  int cub_EB = 0;                     // elements per CTA pass of cubature_relax_kernel
+  double *d_It = nullptr, *d_Pt = nullptr, *d_R = nullptr;
   double *d_xn = nullptr, *d_user_vv = nullptr;
   int32_t *d_EToV = nullptr, *d_vmapP = nullptr;
   int8_t* d_EToB = nullptr;
@@ -94,6 +99,7 @@ void dev_free(T*& p) {
 
 void free_mesh(alegb_ctx* ctx) {
   dev_free(ctx->d_xn); dev_free(ctx->d_user_vv); ctx->coord_mode = ALEGB_COORDS_CLOSED_FORM;
+  dev_free(ctx->d_R); ctx->relax_mode = ALEGB_RELAX_COLLOCATION;
   dev_free(ctx->d_X0); dev_free(ctx->d_xv); dev_free(ctx->d_vv); dev_free(ctx->d_EToV); dev_free(ctx->d_vmapP);
   dev_free(ctx->d_EToB); dev_free(ctx->d_vgeo); dev_free(ctx->d_sgeo); dev_free(ctx->d_vvel);
   dev_free(ctx->d_pml_index); dev_free(ctx->d_pml_elems); dev_free(ctx->d_pml_sigma);
@@ -171,7 +177,17 @@ int check_ready(alegb_ctx* ctx) {
 }
 
 // the fused stage kernel, bracketed by events while profiling is enabled
-int timed_stage(alegb_ctx* ctx, const StageArgs& a, cudaStream_t s) {
+int timed_stage(alegb_ctx* ctx, const StageArgs& a_in, cudaStream_t s) {
+  StageArgs a = a_in;
+  if (ctx->relax_mode == ALEGB_RELAX_CUBATURE) {
+    // kernel v of the paper (L197): R = P N~(I q_in), read by the stage kernel in place of the collocated N~
+    CubArgs cb;
+    cb.K = ctx->K; cb.Np = ctx->ref.Np; cb.Nc = ctx->cub.Nc; cb.EB = ctx->cub_EB;
+    cb.It = ctx->d_It; cb.Pt = ctx->d_Pt; cb.q = a.q_in; cb.R = ctx->d_R; cb.invtau = ctx->invtau;
+    CU(launch_cubature(ctx->ref.dim, cb, ctx->num_sms, s));
+    ctx->launches++;
+    a.relax_cub = ctx->d_R;
+  }
   const bool rec = ctx->profiling && ctx->prof_used + 2 <= 8192;
   if (rec) {
     while (ctx->prof_events.size() < ctx->prof_used + 2) {
@@ -552,6 +568,59 @@ int alegb_set_motion_user(alegb_ctx* ctx, const double* d_xv, const double* d_vv
   CU(cudaStreamSynchronize(0));
   ctx->motion.kind = ALEGB_MOTION_USER;
   ctx->config_version++;
+  return ALEGB_OK;
+}
+
+static int ensure_cubature(alegb_ctx* ctx) {
+  if (ctx->cub.Nc > 0) return ALEGB_OK;
+  std::string err;
+  if (!build_cubature(ctx->ref, 3 * ctx->ref.N, ctx->cub, err)) return fail(ctx, ALEGB_INVALID_ARG, err);
+  return ALEGB_OK;
+}
+
+int alegb_set_relaxation(alegb_ctx* ctx, int mode) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  if (mode != ALEGB_RELAX_COLLOCATION && mode != ALEGB_RELAX_CUBATURE) return fail(ctx, ALEGB_INVALID_ARG, "unknown relaxation mode");
+  if (mode == ALEGB_RELAX_CUBATURE) {
+    if (ctx->device < 0) return fail(ctx, ALEGB_CUDA_ERROR, "host-only context (no CUDA device)");
+    if (!ctx->mesh_ready) return fail(ctx, ALEGB_NOT_READY, "alegb_mesh_upload has not been called");
+    int rc = ensure_cubature(ctx);
+    if (rc != ALEGB_OK) return rc;
+    CU(cudaSetDevice(ctx->device));
+    const int dim = ctx->ref.dim, Np = ctx->ref.Np, Nc = ctx->cub.Nc, NS = dim * (dim + 1) / 2;
+    if (!ctx->d_It) {
+      std::vector<double> It((size_t)Np * Nc), Pt((size_t)Nc * Np);
+      for (int c = 0; c < Nc; ++c) for (int j = 0; j < Np; ++j) {
+        It[(size_t)j * Nc + c] = ctx->cub.I[(size_t)c * Np + j];
+        Pt[(size_t)c * Np + j] = ctx->cub.P[(size_t)j * Nc + c];
+      }
+      CU(dev_alloc(ctx, &ctx->d_It, It.size()));
+      CU(dev_alloc(ctx, &ctx->d_Pt, Pt.size()));
+      CU(cudaMemcpy(ctx->d_It, It.data(), It.size() * sizeof(double), cudaMemcpyHostToDevice));
+      CU(cudaMemcpy(ctx->d_Pt, Pt.data(), Pt.size() * sizeof(double), cudaMemcpyHostToDevice));
+      int EB = 256 / Np;
+      while (EB > 1 && cubature_smem_bytes(dim, Np, Nc, EB) > 200 * 1024) --EB;
+      ctx->cub_EB = EB;
+      CU(configure_cubature(dim, cubature_smem_bytes(dim, Np, Nc, EB)));
+    }
+    if (!ctx->d_R) CU(dev_alloc(ctx, &ctx->d_R, (size_t)ctx->K * NS * Np));
+  }
+  ctx->relax_mode = mode;
+  ctx->config_version++;
+  return ALEGB_OK;
+}
+
+int alegb_get_cubature(alegb_ctx* ctx, int* degree, int* Nc, double* rst, double* w, double* I, double* P) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  int rc = ensure_cubature(ctx);
+  if (rc != ALEGB_OK) return rc;
+  const Cubature& c = ctx->cub;
+  if (degree) *degree = c.degree;
+  if (Nc) *Nc = c.Nc;
+  if (rst) std::memcpy(rst, c.rst.data(), c.rst.size() * sizeof(double));
+  if (w) std::memcpy(w, c.w.data(), c.w.size() * sizeof(double));
+  if (I) std::memcpy(I, c.I.data(), c.I.size() * sizeof(double));
+  if (P) std::memcpy(P, c.P.data(), c.P.size() * sizeof(double));
   return ALEGB_OK;
 }
 

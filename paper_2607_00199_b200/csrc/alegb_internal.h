@@ -46,6 +46,7 @@ struct StageArgs {
   const double* AliftP;  // DMMA path, faces packed along k: [NB][ceil(Nfaces*Nfp/4)][32]
   // physics
   double c, invtau;
+  const double* relax_cub;   // R = P N~(I q) [K][Ns][Np] replacing the collocated N~(q), or NULL (reading R8)
   double q_inf[kMaxFields];
   // fields
   const double* q_in;
@@ -56,6 +57,17 @@ struct StageArgs {
   double* q_out;
   double* acc_out;
   StageCoef coef;
+};
+
+// cubature-projected relaxation (cubature.cu): R[K][Ns][Np] = P N~(I q), Ns = dim (dim+1)/2 stiff fields
+struct CubArgs {
+  int64_t K;
+  int Np, Nc, EB;        // nodes, cubature nodes, elements per CTA pass
+  const double* It;      // [Np][Nc]  I transposed
+  const double* Pt;      // [Nc][Np]  P transposed
+  const double* q;       // [K][Nf][Np]
+  double* R;
+  double invtau;
 };
 
 struct PmlArgs {
@@ -99,6 +111,11 @@ cudaError_t launch_geometry(int dim, int64_t K, const int32_t* EToV, const doubl
 cudaError_t launch_stage(int dim, int N, const StageArgs& a, int num_sms, cudaStream_t s);
 cudaError_t launch_pml(int dim, int N, const PmlArgs& a, int num_sms, cudaStream_t s);
 cudaError_t configure_kernels(int dim, int N);
+
+// cubature-projected relaxation, cubature.cu
+size_t cubature_smem_bytes(int dim, int Np, int Nc, int EB);
+cudaError_t configure_cubature(int dim, size_t smem);
+cudaError_t launch_cubature(int dim, const CubArgs& a, int num_sms, cudaStream_t s);
 
 // tensor-core (DMMA) stage kernel, stage_mma.cu
 struct MmaLayout { int NB, KS, KF; };               // node blocks, k-steps of the volume / per-face contraction

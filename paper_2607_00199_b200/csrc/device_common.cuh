@@ -114,6 +114,22 @@ __device__ __forceinline__ void relaxation(const double* q, double invtau, doubl
   }
 }
 
+// a4 at node n of element e: the collocated N~(q) (reading R8), or -- alegb_set_relaxation(CUBATURE) -- the
+// cubature-projected term R = P N~(I q) that cubature.cu left in a.relax_cub (eq. 9 last term, L197).
+template <int DIM>
+__device__ __forceinline__ void relaxation_term(const StageArgs& a, const double* q, int64_t e, int n, int Np, double* nt) {
+  if (a.relax_cub == nullptr) {
+    relaxation<DIM>(q, a.invtau, nt);
+  } else {
+    constexpr int NS = DIM * (DIM + 1) / 2;
+    const double* r = a.relax_cub + e * NS * Np + n;
+#pragma unroll
+    for (int k = 0; k <= DIM; ++k) nt[k] = 0.0;
+#pragma unroll
+    for (int s = 0; s < NS; ++s) nt[DIM + 1 + s] = __ldg(r + s * Np);
+  }
+}
+
 // Even-moment rows of A^_n applied to a vector w that lives in the first-moment (momentum) slots only.
 template <int DIM>
 __device__ __forceinline__ void normal_apply_odd_to_even(const double* nh, const double* w, double* y) {

@@ -131,6 +131,112 @@ static std::vector<qreal> transpose(const std::vector<qreal>& A, int n, int m) {
   return T;
 }
 
+// Jacobi polynomial P_n^{(a,0)}(x) and its derivative: three-term recurrence and
+// (2n+a)(1-x^2) P_n' = n (a - (2n+a) x) P_n + 2 (n+a) n P_{n-1}   (Abramowitz & Stegun 22.7.1, 22.8.1 with beta = 0)
+static void jacobi_a0(int n, int a, qreal x, qreal& p, qreal& dp) {
+  if (n == 0) { p = 1; dp = 0; return; }
+  qreal p0 = 1, p1 = ((qreal)a + (qreal)(a + 2) * x) / 2;
+  for (int k = 1; k < n; ++k) {
+    const qreal c = 2 * k + a;
+    const qreal A1 = 2 * (qreal)(k + 1) * (k + a + 1) * c;
+    const qreal A2 = (c + 1) * (qreal)(a * a);
+    const qreal A3 = c * (c + 1) * (c + 2);
+    const qreal A4 = 2 * (qreal)(k + a) * k * (c + 2);
+    const qreal pk = ((A2 + A3 * x) * p1 - A4 * p0) / A1;
+    p0 = p1; p1 = pk;
+  }
+  p = p1;
+  dp = (n * ((qreal)a - (qreal)(2 * n + a) * x) * p1 + 2 * (qreal)(n + a) * n * p0) / ((qreal)(2 * n + a) * (1 - x * x));
+}
+
+// n-point Gauss-Jacobi rule for the weight (1-x)^a on [-1,1]: zeros of P_n^{(a,0)} by Newton iteration with
+// deflation, weights w_i = 2^{a+1} / ((1 - x_i^2) P_n'(x_i)^2).  Exact to degree 2n-1.
+static void gauss_jacobi_a0(int n, int a, std::vector<qreal>& x, std::vector<qreal>& w) {
+  x.assign(n, 0); w.assign(n, 0);
+  for (int k = 0; k < n; ++k) {
+    qreal r = -(qreal)cosl(M_PIl * (2 * k + 1) / (2.0L * n));
+    if (k > 0) r = (r + x[k - 1]) / 2;
+    for (int it = 0; it < 200; ++it) {
+      qreal s = 0;
+      for (int j = 0; j < k; ++j) s += 1 / (r - x[j]);
+      qreal p, dp;
+      jacobi_a0(n, a, r, p, dp);
+      const qreal dx = -p / (dp - s * p);
+      r += dx;
+      if (qabs(dx) < (qreal)1e-30L) break;
+    }
+    x[k] = r;
+  }
+  for (int k = 0; k < n; ++k) {
+    qreal p, dp;
+    jacobi_a0(n, a, x[k], p, dp);
+    w[k] = qpow(2, a + 1) / ((1 - x[k] * x[k]) * dp * dp);
+  }
+}
+
+bool build_cubature(const RefElement& ref, int degree, Cubature& out, std::string& err) {
+  const int dim = ref.dim, N = ref.N, Np = ref.Np, nv = dim + 1;
+  if (Np == 0) { err = "reference element not built"; return false; }
+  if (degree < 2 * N) { err = "cubature degree must be at least 2N"; return false; }
+  const int n = degree / 2 + 1;
+  std::vector<qreal> xa, wa, xb, wb, xc, wc;
+  gauss_jacobi_a0(n, 0, xa, wa);
+  gauss_jacobi_a0(n, 1, xb, wb);
+  if (dim == 3) gauss_jacobi_a0(n, 2, xc, wc);
+  // collapsed coordinates: 2-D r = (1+a)(1-b)/2 - 1, s = b, dr ds = (1-b)/2 da db;
+  // 3-D r = (1+a)(1-b)(1-c)/4 - 1, s = (1+b)(1-c)/2 - 1, t = c, dr ds dt = (1-b)(1-c)^2/8 da db dc
+  const int Nc = dim == 2 ? n * n : n * n * n;
+  std::vector<qreal> pts(Nc * dim), wts(Nc);
+  int q = 0;
+  for (int ia = 0; ia < n; ++ia)
+    for (int ib = 0; ib < n; ++ib) {
+      if (dim == 2) {
+        pts[q * 2 + 0] = (1 + xa[ia]) * (1 - xb[ib]) / 2 - 1;
+        pts[q * 2 + 1] = xb[ib];
+        wts[q++] = wa[ia] * wb[ib] / 2;
+      } else {
+        for (int ic = 0; ic < n; ++ic) {
+          pts[q * 3 + 0] = (1 + xa[ia]) * (1 - xb[ib]) * (1 - xc[ic]) / 4 - 1;
+          pts[q * 3 + 1] = (1 + xb[ib]) * (1 - xc[ic]) / 2 - 1;
+          pts[q * 3 + 2] = xc[ic];
+          wts[q++] = wa[ia] * wb[ib] * wc[ic] / 8;
+        }
+      }
+    }
+  // monomial basis in u = (1 + r)/2 as in build_reference: V at the nodes, Vc at the cubature points
+  auto ex = exponents(dim, N);
+  std::vector<qreal> V(Np * Np), Vc(Nc * Np);
+  for (int i = 0; i < Np; ++i)
+    for (int m = 0; m < Np; ++m) {
+      qreal v = 1;
+      for (int d = 0; d < dim; ++d) v *= qpow((qreal)ref.lam[i * nv + d + 1], ex[m][d]);
+      V[i * Np + m] = v;
+    }
+  for (int c = 0; c < Nc; ++c)
+    for (int m = 0; m < Np; ++m) {
+      qreal v = 1;
+      for (int d = 0; d < dim; ++d) v *= qpow((1 + pts[c * dim + d]) / 2, ex[m][d]);
+      Vc[c * Np + m] = v;
+    }
+  std::vector<qreal> Vinv = V;
+  if (!invert(Vinv, Np)) { err = "singular Vandermonde"; return false; }
+  std::vector<qreal> Ginv = gram(dim, ex);
+  if (!invert(Ginv, Np)) { err = "singular Gram matrix"; return false; }
+  std::vector<qreal> Minv = matmul(matmul(V, Ginv, Np, Np, Np), transpose(V, Np, Np), Np, Np, Np);
+  std::vector<qreal> I = matmul(Vc, Vinv, Nc, Np, Np);                      // [Nc][Np]
+  std::vector<qreal> ItW = transpose(I, Nc, Np);                            // [Np][Nc]
+  for (int j = 0; j < Np; ++j) for (int c = 0; c < Nc; ++c) ItW[j * Nc + c] *= wts[c];
+  std::vector<qreal> P = matmul(Minv, ItW, Np, Np, Nc);                     // [Np][Nc]
+  out.degree = degree; out.Nc = Nc;
+  out.rst.resize(dim * Nc); out.w.resize(Nc); out.I.resize(Nc * Np); out.P.resize(Np * Nc);
+  for (int c = 0; c < Nc; ++c) {
+    out.w[c] = (double)wts[c];
+    for (int d = 0; d < dim; ++d) out.rst[d * Nc + c] = (double)pts[c * dim + d];
+  }
+  for (int x = 0; x < Nc * Np; ++x) { out.I[x] = (double)I[x]; out.P[x] = (double)P[x]; }
+  return true;
+}
+
 int RefElement::node_of(const int* wts) const {
   for (int i = 0; i < Np; ++i) {
     bool same = true;

@@ -29,6 +29,18 @@ struct Connectivity {
   std::vector<int32_t> vmapM, vmapP;    // [K][Nfaces][Nfp], flattened node index e*Np+n
 };
 
+// Cubature rule and the interpolation / projection operators of PAPER.md:L84-86, L103:
+// conical-product Gauss-Jacobi rule exact to total degree `degree` on the reference simplex,
+// I_cj = phi_j(x_c), P = M^-1 I^T diag(w) (reference element: the J^e of eq. 9 cancels against (M^e)^-1).
+struct Cubature {
+  int degree = 0, Nc = 0;
+  std::vector<double> rst;   // [dim][Nc]
+  std::vector<double> w;     // [Nc], sum = measure of the reference simplex
+  std::vector<double> I;     // [Nc][Np]
+  std::vector<double> P;     // [Np][Nc]
+};
+bool build_cubature(const RefElement& ref, int degree, Cubature& out, std::string& err);
+
 // Faces matched by (periodic classes of) vertex ids, face nodes by the vertex permutation (never by coordinates).
 // Returns 0, or -2 (BAD_MESH) with err filled.
 int build_connectivity(const RefElement& ref, int64_t K, const int32_t* EToV, const int32_t* vertex_equiv,

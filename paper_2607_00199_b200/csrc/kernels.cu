@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(StageCfg<DIM, N>::Threads) stage_kernel(StageA
 #pragma unroll
       for (int k = 0; k < Nf; ++k) qn[k] = sq[(el * Nf + k) * Np + i];
       double nt[Nf];
-      relaxation<DIM>(qn, a.invtau, nt);  // a4 (L115; reading R8)
+      relaxation_term<DIM>(a, qn, e, i, Np, nt);  // a4 (L115; reading R8, or cubature-projected)
 #pragma unroll
       for (int k = 0; k < Nf; ++k) {
         double v = -c * st[k];

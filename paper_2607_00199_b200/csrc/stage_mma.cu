@@ -170,7 +170,7 @@ __global__ void __launch_bounds__(MmaCfg<DIM, N>::Threads, 1) stage_mma_kernel(S
       hermite_apply<DIM>([&](int d, int j) { return gr[d][j]; }, st);
 #pragma unroll
       for (int k = 0; k < Nf; ++k) qn[k] = qt[(c * Nf + k) * S + nn];
-      relaxation<DIM>(qn, a.invtau, nt);
+      relaxation_term<DIM>(a, qn, e, nn, Np, nt);
 #pragma unroll
       for (int k = 0; k < Nf; ++k) {
         double v = -cs * st[k];

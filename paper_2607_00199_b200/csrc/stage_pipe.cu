@@ -376,7 +376,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
             st);
 #pragma unroll
         for (int k = 0; k < Nf; ++k) qn[k] = qt[(c * Nf + k) * S + nn];
-        relaxation<DIM>(qn, a.invtau, nt);
+        relaxation_term<DIM>(a, qn, e0 + (c < nel ? c : 0), nn, Np, nt);
 #pragma unroll
         for (int k = 0; k < Nf; ++k) {
           double v = fma(-cs, st[k], nt[k]);

@@ -496,3 +496,71 @@ def test_rk_coordinates_user_velocity(refs, B):
     assert np.abs(dx.cpu().numpy() - (xv + 10 * cfg["dt"] * vv)).max() < 1e-15
     assert np.abs(dq.cpu().numpy() - cfg["q0"]).max() < 1e-13       # free stream
     ctx.close()
+
+
+# ------------------------------------------------------------------ NEXT-1: cubature-projected relaxation (L84-107, L197)
+def _cubature_case(name, refs):
+    ref, cfg = make_case(name, refs)
+    cfg["relax"] = "cubature"
+    return ref, cfg, oracle_problem(cfg, ref)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "tri_N5", "tet_N2"])
+def test_cubature_rhs_matches_oracle(name, kernel, refs, B):
+    ref, cfg, P = _cubature_case(name, refs)
+    ctx = make_ctx(B, cfg, kernel)
+    ctx.alegb_set_relaxation(B.RELAX_CUBATURE)
+    q = perturbed(cfg, amp=3e-2)                     # large enough for the projection to differ from collocation
+    dq, dF = dev(q), torch.empty(q.shape, dtype=torch.float64, device="cuda")
+    t = 0.31
+    ctx.alegb_rhs(t, dq, dF)
+    torch.cuda.synchronize()
+    out = P.rhs(q, t, want_abs=True)
+    F, Fabs = out[0], out[-1]
+    assert (np.abs(dF.cpu().numpy() - F) <= TOL_F * (Fabs + 1e-3 * Fabs.max())).all()
+    # the mode is live: the collocated operator differs by far more than the tolerance
+    ctx.alegb_set_relaxation(B.RELAX_COLLOCATION)
+    dF2 = torch.empty_like(dF)
+    ctx.alegb_rhs(t, dq, dF2)
+    torch.cuda.synchronize()
+    assert (dF2 - dF).abs().max().item() > 1e3 * TOL_F * Fabs.max()
+    ctx.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", ["cfg1", "cfg3", "cfg4"])
+def test_cubature_stage_states_and_steps_match_oracle(name, refs, B):
+    ref, cfg, P = _cubature_case(name, refs)
+    ctx = B.context_from_config(cfg)
+    ctx.alegb_set_relaxation(B.RELAX_CUBATURE)
+    q = perturbed(cfg)
+    st = torch.empty((4,) + q.shape, dtype=torch.float64, device="cuda")
+    ctx.alegb_step_debug(dev(q), 0.1, cfg["dt"], st)
+    torch.cuda.synchronize()
+    so, _ = sark.step_debug(P, q, 0.1, cfg["dt"])
+    for i in range(4):
+        assert rel_linf(st[i].cpu().numpy(), so[i]) <= TOL_STAGE
+    # 20 steps through the captured graph (alegb_step_debug advanced the library's PML state: start it from zero)
+    if P.sigma is not None:
+        ctx.alegb_pml_reset()
+    dq = dev(q)
+    ctx.alegb_step(dq, 0.0, cfg["dt"], 20)
+    torch.cuda.synchronize()
+    qo = sark.step(P, q, 0.0, cfg["dt"], 20)
+    qo = qo[0] if isinstance(qo, tuple) else qo
+    assert rel_linf(dq.cpu().numpy(), qo) <= TOL_100
+    ctx.close()
+
+
+@pytest.mark.gpu
+def test_cubature_free_stream_on_gpu(refs, B):
+    ref, cfg = make_case("cfg1", refs)
+    ctx = B.context_from_config(cfg)
+    ctx.alegb_set_relaxation(B.RELAX_CUBATURE)
+    dq = dev(cfg["q0"])
+    ctx.alegb_step(dq, 0.0, cfg["dt"], 50)
+    torch.cuda.synchronize()
+    assert np.abs(dq.cpu().numpy() - cfg["q0"]).max() < 1e-13
+    ctx.close()

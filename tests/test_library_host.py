@@ -210,3 +210,33 @@ def test_sark_coefficients_against_oracle_and_identities(gamma):
         assert abs(b.sum() - phi(gamma)) < 1e-15
     else:
         assert list(a) == [0.5, 0.0, 0.5, 0.0, 0.0, 1.0] and np.allclose(b, [1 / 6, 1 / 3, 1 / 3, 1 / 6], atol=0, rtol=1e-16)
+
+
+@pytest.mark.parametrize("dim,N", [(2, 1), (2, 3), (2, 4), (2, 5), (3, 2), (3, 3), (3, 4), (3, 5)])
+def test_cubature_matches_oracle_and_integrates_exactly(dim, N, refs):
+    """NEXT-1: the library's own Gauss-Jacobi rule, I and P (host_ref.cpp, __float128, monomial
+    basis) against the oracle's (scipy roots, product-Legendre basis), and against Dirichlet's closed-form integrals."""
+    from math import factorial
+    from oracle.cubature import Cubature
+    from paper_2607_00199_b200 import binding as B
+    ctx = B.Context(dim, N, -1)
+    got = ctx.alegb_get_cubature()
+    ref = refs(dim, N)
+    cub = Cubature(ref)
+    assert got["degree"] == 3 * N and got["Nc"] == cub.Nc
+    # the two rules may order their points differently: sort both lexicographically
+    def order(x):
+        return np.lexsort(np.round(x.T[::-1], 12))
+    og, oo = order(got["rst"].T), order(cub.x)
+    assert np.abs(got["rst"].T[og] - cub.x[oo]).max() < 1e-14
+    assert np.abs(got["w"][og] - cub.w[oo]).max() < 1e-15
+    assert np.abs(got["I"][og] - cub.I[oo]).max() < 1e-12
+    assert np.abs(got["P"][:, og] - cub.P[:, oo]).max() < 1e-12
+    # closed form: sum_c w_c prod ((1+x_d)/2)^e_d = 2^dim prod e_d! / (sum e + dim)!
+    x, w = got["rst"].T, got["w"]
+    rng = np.random.default_rng(199)
+    for _ in range(20):
+        e = rng.multinomial(3 * N, np.ones(dim + 1) / (dim + 1))[:dim]
+        exact = 2.0 ** dim * np.prod([factorial(int(v)) for v in e]) / factorial(int(e.sum()) + dim)
+        assert abs(w @ np.prod(((1 + x) / 2) ** e, axis=1) - exact) < 1e-15
+    ctx.close()
