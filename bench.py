@@ -40,7 +40,7 @@ HBM_FALLBACK_GBS = 6650.0
 ALGO_BYTES_PER_DOF_STAGE = 38.0          # 152 B per DOF-step
 POINTWISE_FLOP_PER_DOF_STAGE = 50.0
 # dram__bytes_read.sum + dram__bytes_write.sum of the stage kernel per launch from the committed `ncu --set full`
-# capture (mean over the four stages of a step: 1.79 / 2.93 / 3.48 / 1.82 GB), profiles/r1_v3_pipe_stage_kernel.md
+# capture (mean over the four stages of a step: 1.79 / 2.93 / 3.48 / 1.82 GB), profiles/r1_v8_pipe_stage_kernel.md
 NCU_DRAM_BYTES_PER_LAUNCH = {4: 2.505e9}
 
 
@@ -190,6 +190,10 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--kernel", type=int, default=0, choices=[0, 1, 2, 3],
                     help="alegb_set_kernel: 0 auto, 1 generic DFMA, 2 pipelined DMMA, 3 warp-per-quad DMMA")
+    ap.add_argument("--relax", default="collocation", choices=["collocation", "cubature"],
+                    help="nonlinear relaxation: collocated (default, DESIGN.md R8) or cubature-projected (NEXT-1)")
+    ap.add_argument("--coords", default="closed", choices=["closed", "rk"],
+                    help="vertex positions: closed-form law (default, R9) or advanced by the solver's RK4 (NEXT-2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -218,6 +222,10 @@ def main():
     cfg = make_config(args.config, lam)
     ctx = B.context_from_config(cfg, local_rank)
     ctx.alegb_set_kernel(args.kernel)
+    if args.relax == "cubature":
+        ctx.alegb_set_relaxation(B.RELAX_CUBATURE)
+    if args.coords == "rk":
+        ctx.alegb_set_coordinate_mode(B.COORDS_RK, 0.0)
     K, Np, Nf, Nfp = cfg["K"], cfg["Np"], cfg["Nf"], ctx.Nfp
     dof = K * Np * Nf
     dt = cfg["dt"]
@@ -293,7 +301,7 @@ def main():
     roofline = dict(roofline)
     if args.kernel == 0:
         roofline["traffic"] = NCU_DRAM_BYTES_PER_LAUNCH.get(args.config)
-        roofline["traffic_unit"] = "bytes per launch (ncu dram read+write, profiles/r1_v3_pipe_stage_kernel.md)"
+        roofline["traffic_unit"] = "bytes per launch (ncu dram read+write, profiles/r1_v8_pipe_stage_kernel.md)"
         roofline["algorithmic_bytes_per_launch"] = dof * ALGO_BYTES_PER_DOF_STAGE
     roofline.update({"kernel": "alegb stage kernel (fused volume+relaxation+surface+SARK update)",
                      "kernel_ms": kern_ms, "kernel_launches_timed": nprof,
@@ -309,7 +317,7 @@ def main():
                        "dt": dt, "parallelism": "replicas x%d (north_star: one GPU, no sharding)" % world,
                        "l2": "state arrays are %.0f MB each (> 126 MB L2), no flush needed" % (state_bytes / 1e6)
                        if state_bytes > 200e6 else "state is L2-resident (%.1f MB); launch-latency bound" % (state_bytes / 1e6),
-                       "state_finite": finite, "kernel": args.kernel,
+                       "state_finite": finite, "kernel": args.kernel, "relax": args.relax, "coords": args.coords,
                        "launch": "one CUDA graph per step" if graph_timed and args.steps >= 2 else "direct launches"},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
 

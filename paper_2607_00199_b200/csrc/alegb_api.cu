@@ -37,6 +37,7 @@ struct alegb_ctx {
   Cubature cub;                       // host copy (built on first use)
   int cub_EB = 0;                     // elements per CTA pass of cubature_relax_kernel
   double *d_It = nullptr, *d_Pt = nullptr, *d_R = nullptr;
+  double *d_AI = nullptr, *d_AP = nullptr;   // I, P in DMMA A-fragment order (cubature_mma_kernel)
   double *d_xn = nullptr, *d_user_vv = nullptr;
   int32_t *d_EToV = nullptr, *d_vmapP = nullptr;
   int8_t* d_EToB = nullptr;
@@ -183,8 +184,11 @@ int timed_stage(alegb_ctx* ctx, const StageArgs& a_in, cudaStream_t s) {
     // kernel v of the paper (L197): R = P N~(I q_in), read by the stage kernel in place of the collocated N~
     CubArgs cb;
     cb.K = ctx->K; cb.Np = ctx->ref.Np; cb.Nc = ctx->cub.Nc; cb.EB = ctx->cub_EB;
-    cb.It = ctx->d_It; cb.Pt = ctx->d_Pt; cb.q = a.q_in; cb.R = ctx->d_R; cb.invtau = ctx->invtau;
-    CU(launch_cubature(ctx->ref.dim, cb, ctx->num_sms, s));
+    cb.It = ctx->d_It; cb.Pt = ctx->d_Pt; cb.AI = ctx->d_AI; cb.AP = ctx->d_AP;
+    cb.q = a.q_in; cb.R = ctx->d_R; cb.invtau = ctx->invtau;
+    // kernel kind 1 (generic DFMA stage kernel) keeps the DFMA cubature kernel: two independent implementations
+    if (ctx->kernel_mode == 1) CU(launch_cubature(ctx->ref.dim, cb, ctx->num_sms, s));
+    else CU(launch_cubature_mma(ctx->ref.dim, ctx->ref.N, cb, ctx->num_sms, s));
     ctx->launches++;
     a.relax_cub = ctx->d_R;
   }
@@ -598,6 +602,23 @@ int alegb_set_relaxation(alegb_ctx* ctx, int mode) {
       CU(dev_alloc(ctx, &ctx->d_Pt, Pt.size()));
       CU(cudaMemcpy(ctx->d_It, It.data(), It.size() * sizeof(double), cudaMemcpyHostToDevice));
       CU(cudaMemcpy(ctx->d_Pt, Pt.data(), Pt.size() * sizeof(double), cudaMemcpyHostToDevice));
+      {   // A-fragment order: lane l of fragment (row tile, k-step) holds A[8 tile + l/4][4 k + l%4], zero outside
+        int NRT, KS, NB;
+        cubature_mma_layout(dim, ctx->ref.N, NRT, KS, NB);
+        std::vector<double> AI((size_t)NRT * KS * 32, 0.0), AP((size_t)NB * 2 * NRT * 32, 0.0);
+        for (int rt = 0; rt < NRT; ++rt) for (int ks = 0; ks < KS; ++ks) for (int l = 0; l < 32; ++l) {
+          const int row = 8 * rt + l / 4, col = 4 * ks + l % 4;
+          if (row < Nc && col < Np) AI[((size_t)rt * KS + ks) * 32 + l] = ctx->cub.I[(size_t)row * Np + col];
+        }
+        for (int r = 0; r < NB; ++r) for (int k = 0; k < 2 * NRT; ++k) for (int l = 0; l < 32; ++l) {
+          const int row = 8 * r + l / 4, col = 4 * k + l % 4;
+          if (row < Np && col < Nc) AP[((size_t)r * 2 * NRT + k) * 32 + l] = ctx->cub.P[(size_t)row * Nc + col];
+        }
+        CU(dev_alloc(ctx, &ctx->d_AI, AI.size()));
+        CU(dev_alloc(ctx, &ctx->d_AP, AP.size()));
+        CU(cudaMemcpy(ctx->d_AI, AI.data(), AI.size() * sizeof(double), cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(ctx->d_AP, AP.data(), AP.size() * sizeof(double), cudaMemcpyHostToDevice));
+      }
       int EB = 256 / Np;
       while (EB > 1 && cubature_smem_bytes(dim, Np, Nc, EB) > 200 * 1024) --EB;
       ctx->cub_EB = EB;

@@ -65,6 +65,8 @@ struct CubArgs {
   int Np, Nc, EB;        // nodes, cubature nodes, elements per CTA pass
   const double* It;      // [Np][Nc]  I transposed
   const double* Pt;      // [Nc][Np]  P transposed
+  const double* AI;      // DMMA path: I in A-fragment order [NRT][KS][32]
+  const double* AP;      // DMMA path: P in A-fragment order [NB][2 NRT][32]
   const double* q;       // [K][Nf][Np]
   double* R;
   double invtau;
@@ -116,6 +118,8 @@ cudaError_t configure_kernels(int dim, int N);
 size_t cubature_smem_bytes(int dim, int Np, int Nc, int EB);
 cudaError_t configure_cubature(int dim, size_t smem);
 cudaError_t launch_cubature(int dim, const CubArgs& a, int num_sms, cudaStream_t s);
+void cubature_mma_layout(int dim, int N, int& NRT, int& KS, int& NB);   // fragment-array extents
+cudaError_t launch_cubature_mma(int dim, int N, const CubArgs& a, int num_sms, cudaStream_t s);   // InvalidValue: none for (dim, N)
 
 // tensor-core (DMMA) stage kernel, stage_mma.cu
 struct MmaLayout { int NB, KS, KF; };               // node blocks, k-steps of the volume / per-face contraction

@@ -96,4 +96,161 @@ cudaError_t launch_cubature(int dim, const CubArgs& a, int num_sms, cudaStream_t
   return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// Tensor-core version (DMMA, mma.sync.m8n8k4.f64).  One warp owns a quad of 4 consecutive elements from start to end;
+// no shared-memory operand tiles, no block-level synchronisation:
+//   * I and P are stored in A-fragment order (lane l of fragment (row tile, k-step) holds A[8 tile + l/4][4 k + l%4]),
+//     so an operand is one coalesced 256-byte load; both matrices (99 + 110 kB at 3-D N = 4) are shared by every warp
+//     of the SM and live in L1 (the kernel uses < 13 kB of shared memory);
+//   * the quad's input fields are the B operand of the interpolation and stay in registers for all row tiles:
+//     column g <-> (element g/2, field 2t + g%2) as in stage_pipe.cu, so after the contraction lane (g, c) holds
+//     q1 .. q_{1+dim} of element c at cubature node 8 rt + g and evaluates N~ there (L115);
+//   * the projection is a K-accumulation over the cubature nodes, so it is fused block by block: the 8 nodes of a row
+//     tile are 2 k-steps of P N~; N~ goes through a 2 kB warp-private staging tile to become a B fragment;
+//   * the result leaves the accumulators in the layout of the stage kernels (lane = node, element).
+template <int DIM, int N>
+struct CubCfg {
+  static constexpr int Np = DIM == 2 ? (N + 1) * (N + 2) / 2 : (N + 1) * (N + 2) * (N + 3) / 6;
+  static constexpr int NQ = 3 * N / 2 + 1;                       // Gauss-Jacobi points per direction, degree 3N
+  static constexpr int Nc = DIM == 2 ? NQ * NQ : NQ * NQ * NQ;
+  static constexpr int NRT = (Nc + 7) / 8;                       // row tiles of the interpolation = blocks of 8 nodes
+  static constexpr int KS = (Np + 3) / 4;                        // k-steps of the interpolation
+  static constexpr int NB = (Np + 7) / 8;                        // row tiles of the projection
+  static constexpr int NS = DIM * (DIM + 1) / 2;                 // stiff fields
+  static constexpr int NT2 = (NS + 1) / 2;                       // column tiles of the projection (field pairs)
+  static constexpr int NSP = 2 * NT2;
+  static constexpr int ST = 10;                                  // staging row stride (doubles)
+  static constexpr int Warps = 8;
+  static constexpr int stage_doubles = 4 * NSP * ST;
+  static constexpr size_t smem_bytes = (size_t)Warps * stage_doubles * 8;
+};
+
+__device__ __forceinline__ void cub_dmma(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+               : "+d"(c0), "+d"(c1)
+               : "d"(a), "d"(b));
+}
+
+template <int DIM, int N>
+__global__ void __launch_bounds__(CubCfg<DIM, N>::Warps * 32) cubature_mma_kernel(CubArgs a) {
+  using C = CubCfg<DIM, N>;
+  constexpr int Np = C::Np, Nc = C::Nc, NRT = C::NRT, KS = C::KS, NB = C::NB, NS = C::NS, NT2 = C::NT2, NSP = C::NSP;
+  constexpr int ST = C::ST, Nf = DIM == 2 ? 6 : 10;
+  extern __shared__ double sm[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, c = lane & 3;
+  double* sN = sm + warp * C::stage_doubles;              // [4 elements x NSP fields][ST]: N~ at the 8 nodes of a block
+  for (int x = lane; x < C::stage_doubles; x += 32) sN[x] = 0.0;
+  __syncwarp();
+  const int64_t nquads = (a.K + 3) / 4;
+  for (int64_t quad = (int64_t)blockIdx.x * C::Warps + warp; quad < nquads; quad += (int64_t)gridDim.x * C::Warps) {
+    const int64_t e0 = quad * 4;
+    const int nel = (a.K - e0) < 4 ? (int)(a.K - e0) : 4;
+    // B operand of the interpolation, two column tiles: tile t, column g <-> (element g/2, field 2t + g%2); k = c
+    double bq[KS][2];
+    {
+      const int eb = (g >> 1) < nel ? (g >> 1) : 0;
+#pragma unroll
+      for (int t = 0; t < 2; ++t) {
+        const int f = 2 * t + (g & 1);
+        const double* src = a.q + ((e0 + eb) * Nf + (f <= DIM ? f : 0)) * Np;
+#pragma unroll
+        for (int ks = 0; ks < KS; ++ks) {
+          const int j = 4 * ks + c;
+          bq[ks][t] = (f <= DIM && j < Np) ? __ldg(src + j) : 0.0;
+        }
+      }
+    }
+    double acc2[NB][NT2][2];
+#pragma unroll
+    for (int r = 0; r < NB; ++r)
+#pragma unroll
+      for (int t = 0; t < NT2; ++t) acc2[r][t][0] = acc2[r][t][1] = 0.0;
+#pragma unroll 1
+    for (int rt = 0; rt < NRT; ++rt) {
+      // ---- interpolation to the 8 cubature nodes of this block (L86): lane (g, c) <- node 8 rt + g, element c
+      double i0[2] = {0.0, 0.0}, i1[2] = {0.0, 0.0};
+      const double* ai = a.AI + ((size_t)rt * KS) * 32 + lane;
+#pragma unroll
+      for (int ks = 0; ks < KS; ++ks) {
+        const double af = __ldg(ai + ks * 32);
+        cub_dmma(i0[0], i0[1], af, bq[ks][0]);
+        cub_dmma(i1[0], i1[1], af, bq[ks][1]);
+      }
+      // ---- N~ at the node (L115)
+      double qq[Nf], nt[Nf];
+#pragma unroll
+      for (int f = 0; f < Nf; ++f) qq[f] = 0.0;
+      qq[0] = i0[0]; qq[1] = i0[1]; qq[2] = i1[0];
+      if constexpr (DIM == 3) qq[3] = i1[1];
+      const bool pvalid = 8 * rt + g < Nc;
+      if (!pvalid) qq[0] = 1.0;                           // padding node: any finite value, its P column is zero
+      relaxation<DIM>(qq, a.invtau, nt);
+      __syncwarp();
+#pragma unroll
+      for (int s = 0; s < NS; ++s) sN[(c * NSP + s) * ST + g] = pvalid ? nt[DIM + 1 + s] : 0.0;
+      __syncwarp();
+      // ---- projection, K-accumulated over this block's 2 k-steps (L103)
+#pragma unroll
+      for (int k2 = 0; k2 < 2; ++k2) {
+        double bf[NT2];
+#pragma unroll
+        for (int t = 0; t < NT2; ++t) bf[t] = sN[((g >> 1) * NSP + 2 * t + (g & 1)) * ST + 4 * k2 + c];
+        const double* ap = a.AP + ((size_t)(2 * rt + k2)) * 32 + lane;
+#pragma unroll
+        for (int r = 0; r < NB; ++r) {
+          const double af = __ldg(ap + (size_t)r * (2 * NRT) * 32);
+#pragma unroll
+          for (int t = 0; t < NT2; ++t) cub_dmma(acc2[r][t][0], acc2[r][t][1], af, bf[t]);
+        }
+      }
+    }
+    // ---- store: lane (g, c) holds node 8 r + g of element c, fields 2t, 2t+1
+    if (c < nel) {
+#pragma unroll
+      for (int r = 0; r < NB; ++r) {
+        const int i = 8 * r + g;
+        if (i < Np) {
+#pragma unroll
+          for (int t = 0; t < NT2; ++t)
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+              if (2 * t + h < NS) a.R[((e0 + c) * NS + 2 * t + h) * Np + i] = acc2[r][t][h];
+        }
+      }
+    }
+  }
+}
+
+template <int DIM, int N>
+static cudaError_t launch_cub_mma_one(const CubArgs& a, int num_sms, cudaStream_t s) {
+  using C = CubCfg<DIM, N>;
+  const int64_t nquads = (a.K + 3) / 4;
+  if (nquads == 0) return cudaSuccess;
+  const int64_t want = (nquads + C::Warps - 1) / C::Warps;
+  const int64_t cap = (int64_t)num_sms * 2;
+  cubature_mma_kernel<DIM, N><<<(int)(want < cap ? want : cap), C::Warps * 32, C::smem_bytes, s>>>(a);
+  return cudaGetLastError();
+}
+
+void cubature_mma_layout(int dim, int N, int& NRT, int& KS, int& NB) {
+  const int Np = dim == 2 ? (N + 1) * (N + 2) / 2 : (N + 1) * (N + 2) * (N + 3) / 6;
+  const int NQ = 3 * N / 2 + 1, Nc = dim == 2 ? NQ * NQ : NQ * NQ * NQ;
+  NRT = (Nc + 7) / 8; KS = (Np + 3) / 4; NB = (Np + 7) / 8;
+}
+
+cudaError_t launch_cubature_mma(int dim, int N, const CubArgs& a, int num_sms, cudaStream_t s) {
+  switch (dim * 10 + N) {
+    case 21: return launch_cub_mma_one<2, 1>(a, num_sms, s);
+    case 22: return launch_cub_mma_one<2, 2>(a, num_sms, s);
+    case 23: return launch_cub_mma_one<2, 3>(a, num_sms, s);
+    case 24: return launch_cub_mma_one<2, 4>(a, num_sms, s);
+    case 25: return launch_cub_mma_one<2, 5>(a, num_sms, s);
+    case 31: return launch_cub_mma_one<3, 1>(a, num_sms, s);
+    case 32: return launch_cub_mma_one<3, 2>(a, num_sms, s);
+    case 33: return launch_cub_mma_one<3, 3>(a, num_sms, s);
+    case 34: return launch_cub_mma_one<3, 4>(a, num_sms, s);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
 }  // namespace alegb
