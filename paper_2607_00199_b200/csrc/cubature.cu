@@ -97,6 +97,12 @@ cudaError_t launch_cubature(int dim, const CubArgs& a, int num_sms, cudaStream_t
 }
 
 // ------------------------------------------------------------------------------------------------------------------
+#ifndef ALEGB_CUB_MINB
+#define ALEGB_CUB_MINB 1
+#endif
+#ifndef ALEGB_CUB_WARPS
+#define ALEGB_CUB_WARPS 12   // 3 per SM sub-partition (up to 168 registers); 8: 20.1, 16: 22.4, 12: 22.9 GDOF-stage/s on config 4
+#endif
 // Tensor-core version (DMMA, mma.sync.m8n8k4.f64).  One warp owns a quad of 4 consecutive elements from start to end;
 // no shared-memory operand tiles, no block-level synchronisation:
 //   * I and P are stored in A-fragment order (lane l of fragment (row tile, k-step) holds A[8 tile + l/4][4 k + l%4]),
@@ -120,7 +126,7 @@ struct CubCfg {
   static constexpr int NT2 = (NS + 1) / 2;                       // column tiles of the projection (field pairs)
   static constexpr int NSP = 2 * NT2;
   static constexpr int ST = 10;                                  // staging row stride (doubles)
-  static constexpr int Warps = 8;
+  static constexpr int Warps = ALEGB_CUB_WARPS;
   static constexpr int stage_doubles = 4 * NSP * ST;
   static constexpr size_t smem_bytes = (size_t)Warps * stage_doubles * 8;
 };
@@ -132,7 +138,7 @@ __device__ __forceinline__ void cub_dmma(double& c0, double& c1, double a, doubl
 }
 
 template <int DIM, int N>
-__global__ void __launch_bounds__(CubCfg<DIM, N>::Warps * 32) cubature_mma_kernel(CubArgs a) {
+__global__ void __launch_bounds__(CubCfg<DIM, N>::Warps * 32, ALEGB_CUB_MINB) cubature_mma_kernel(CubArgs a) {
   using C = CubCfg<DIM, N>;
   constexpr int Np = C::Np, Nc = C::Nc, NRT = C::NRT, KS = C::KS, NB = C::NB, NS = C::NS, NT2 = C::NT2, NSP = C::NSP;
   constexpr int ST = C::ST, Nf = DIM == 2 ? 6 : 10;
@@ -227,7 +233,7 @@ static cudaError_t launch_cub_mma_one(const CubArgs& a, int num_sms, cudaStream_
   const int64_t nquads = (a.K + 3) / 4;
   if (nquads == 0) return cudaSuccess;
   const int64_t want = (nquads + C::Warps - 1) / C::Warps;
-  const int64_t cap = (int64_t)num_sms * 2;
+  const int64_t cap = (int64_t)num_sms * ALEGB_CUB_MINB;
   cubature_mma_kernel<DIM, N><<<(int)(want < cap ? want : cap), C::Warps * 32, C::smem_bytes, s>>>(a);
   return cudaGetLastError();
 }
