@@ -19,8 +19,10 @@ Modules
   physics     Hermite-moment system matrices, collision terms, upwind matrices (L36-53, L79-84, L115)
   rhs         F(q,t) = L(q) + N~(q) of eq. 9/10 on the moved mesh (L107, L113-117)
   sark        SARK4 coefficients (L148) and the stage recurrence (L132-134)
+  cubature    cubature-projected relaxation P N~(I q) of eq. 9 / kernel v (L84-107, L197)
+  coords      vertex coordinates advanced by the solver's RK4 (L152, L233)
 
-Parity status: every function here is pinned by ``tests/test_oracle_*.py`` (-m "not gpu") except the wall /
+Parity status: every function here (cubature.py and coords.py included) is pinned by ``tests/test_oracle_*.py`` (-m "not gpu") except the wall /
 far-field boundary states and the PML terms, whose *equations* the paper never prints (PAPER.md:L5, L371 name the
 PML only; boundary conditions are not stated).  Those two carry "parity unpinned by the paper" in rhs.py and
 DESIGN.md: they are pinned only by invariants (uniform-state preservation, sigma=0 reduction, damping).
