@@ -182,13 +182,31 @@ template <int DIM>
 __device__ __forceinline__ void upwind_flux(const double* qM, const double* qP, const double* nh, double c, double vn,
                                             double Fscale, double* fl) {
   constexpr int Nf = DIM == 2 ? 6 : 10;
-  double dq[Nf], y1[Nf], absA[Nf];
+  // (|A^_n| - A^_n)[q] without forming either: with y = (A^_n [q])_odd = B^T [q]_even (see abs_normal_apply)
+  //   odd rows :  [q]_odd + (sqrt3 - 1)(n . [q]_odd) n - y
+  //   even rows:  B ( y + (1/sqrt3 - 1)(n . y) n ) - B [q]_odd  =  B ( y + (1/sqrt3 - 1)(n . y) n - [q]_odd )
+  double dq[Nf], y1[Nf], r[Nf];
 #pragma unroll
   for (int k = 0; k < Nf; ++k) dq[k] = qP[k] - qM[k];
-  abs_normal_apply<DIM>(nh, dq, y1, absA);
-  const double vp = fmax(vn, 0.0), hc = 0.5 * c;
+  normal_apply<DIM>(nh, dq, y1);   // only the odd rows 1..DIM are used; the rest is dead code
+  double nm = 0.0, ny = 0.0;
 #pragma unroll
-  for (int k = 0; k < Nf; ++k) fl[k] = Fscale * fma(hc, absA[k] - y1[k], vp * dq[k]);
+  for (int d = 0; d < DIM; ++d) {
+    nm = fma(nh[d], dq[1 + d], nm);
+    ny = fma(nh[d], y1[1 + d], ny);
+  }
+  nm *= ALEGB_SQRT3 - 1.0;
+  ny *= 1.0 / ALEGB_SQRT3 - 1.0;
+  double z[DIM];
+#pragma unroll
+  for (int d = 0; d < DIM; ++d) {
+    r[1 + d] = fma(nm, nh[d], dq[1 + d]) - y1[1 + d];
+    z[d] = fma(ny, nh[d], y1[1 + d]) - dq[1 + d];
+  }
+  normal_apply_odd_to_even<DIM>(nh, z, r);
+  const double hcF = Fscale * (0.5 * c), vpF = Fscale * fmax(vn, 0.0);
+#pragma unroll
+  for (int k = 0; k < Nf; ++k) fl[k] = fma(hcF, r[k], vpF * dq[k]);
 }
 
 // Directional piece of the flux for the absorbing layer (reading R12):
