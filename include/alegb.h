@@ -126,6 +126,14 @@ int alegb_set_relaxation(alegb_ctx* ctx, int mode);
  * I[Nc][Np] (L86), P[Np][Nc] (L103).  Call with the arrays NULL first to learn Nc.  Works on host-only contexts. */
 int alegb_get_cubature(alegb_ctx* ctx, int* degree, int* Nc, double* rst, double* w, double* I, double* P);
 
+/* Pressure and viscous force on the faces tagged `tag` (1 = wall) at time t:
+ *   F_p = - int p n_b dS,  F_v = int sigma . n_b dS,  p = q1 RT (L53), sigma from the second moments (L51),
+ *   n_b = outward normal of the body, face integrals by the nodal face quadrature sJ (1^T M^f) (reading R22);
+ * c_D = F_x / (0.5 rho u^2 c) etc. are the caller's division.  DEVICE q [K][Nf][Np]; HOST out h_Fp[dim], h_Fv[dim].
+ * Geometry from the closed-form law at t.  Enqueues on `stream` and synchronises it.  Deterministic (fixed grid,
+ * ordered second pass).  A mesh without tagged faces gives zeros.  Errors: INVALID_ARG, NOT_READY, CUDA_ERROR. */
+int alegb_wall_forces(alegb_ctx* ctx, double t, const double* d_q, int tag, double* h_Fp, double* h_Fv, void* stream);
+
 /* Select the coordinate mode.  RK: the library's current positions x_n are set to the law's positions at t_start
  * (kind USER: to the positions last given to alegb_set_motion_user); every alegb_step then advances them, so
  * consecutive calls must continue in time where the previous one ended.  alegb_step_debug reads x_n and leaves it

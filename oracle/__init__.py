@@ -21,6 +21,7 @@ Modules
   sark        SARK4 coefficients (L148) and the stage recurrence (L132-134)
   cubature    cubature-projected relaxation P N~(I q) of eq. 9 / kernel v (L84-107, L197)
   coords      vertex coordinates advanced by the solver's RK4 (L152, L233)
+  forces      pressure / viscous force integrals on wall faces (L308, L369 with L51, L53)
 
 Parity status: every function here (cubature.py and coords.py included) is pinned by ``tests/test_oracle_*.py`` (-m "not gpu") except the wall /
 far-field boundary states and the PML terms, whose *equations* the paper never prints (PAPER.md:L5, L371 name the

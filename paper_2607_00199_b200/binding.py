@@ -34,6 +34,7 @@ _SIGNATURES = {
     "alegb_set_motion_user": (_c.c_int, [_P, _P, _P]),
     "alegb_set_coordinate_mode": (_c.c_int, [_P, _c.c_int, _c.c_double]),
     "alegb_set_relaxation": (_c.c_int, [_P, _c.c_int]),
+    "alegb_wall_forces": (_c.c_int, [_P, _c.c_double, _P, _c.c_int, _P, _P, _P]),
     "alegb_get_cubature": (_c.c_int, [_P, _c.POINTER(_c.c_int), _c.POINTER(_c.c_int), _P, _P, _P, _P]),
     "alegb_get_positions": (_c.c_int, [_P, _P, _P]),
     "alegb_rhs": (_c.c_int, [_P, _c.c_double, _P, _P, _P]),
@@ -145,6 +146,12 @@ class Context:
 
     def alegb_set_motion_user(self, d_xv, d_vv):
         self._check(_lib.alegb_set_motion_user(self._h, _dev(d_xv), _dev(d_vv)))
+
+    def alegb_wall_forces(self, t, d_q, tag=1, stream=None):
+        """-> (F_p[dim], F_v[dim]) host arrays."""
+        Fp, Fv = np.zeros(self.dim), np.zeros(self.dim)
+        self._check(_lib.alegb_wall_forces(self._h, float(t), _dev(d_q), int(tag), Fp.ctypes.data, Fv.ctypes.data, _stream(stream)))
+        return Fp, Fv
 
     def alegb_set_relaxation(self, mode):
         self._check(_lib.alegb_set_relaxation(self._h, int(mode)))

@@ -24,6 +24,7 @@ struct alegb_ctx {
   // device: operators
   double *d_Dt = nullptr, *d_LIFTt = nullptr, *d_lam = nullptr, *d_Avol = nullptr, *d_Alift = nullptr, *d_AliftP = nullptr;
   int32_t* d_fmask = nullptr;
+  double *d_wface = nullptr, *d_force = nullptr;   // NEXT-3: face quadrature weights; partial sums + result
   bool mma_ok = false;   // a warp-per-quad DMMA stage kernel exists for (dim, N)
   bool pipe_ok = false;  // a pipelined DMMA stage kernel exists for (dim, N)
   bool pml_mma_ok = false;  // a DMMA kernel for the absorbing layer's auxiliary fields exists for (dim, N)
@@ -411,7 +412,8 @@ int alegb_create(alegb_ctx** out, int dim, int N, int cuda_device) {
   if (upload(ctx, &ctx->d_Dt, Dt.data(), Dt.size()) != cudaSuccess ||
       upload(ctx, &ctx->d_LIFTt, Lt.data(), Lt.size()) != cudaSuccess ||
       upload(ctx, &ctx->d_lam, r.lam.data(), r.lam.size()) != cudaSuccess ||
-      upload(ctx, &ctx->d_fmask, fm.data(), fm.size()) != cudaSuccess) {
+      upload(ctx, &ctx->d_fmask, fm.data(), fm.size()) != cudaSuccess ||
+      upload(ctx, &ctx->d_wface, r.wface.data(), r.wface.size()) != cudaSuccess) {
     alegb_destroy(ctx);
     return ALEGB_CUDA_ERROR;
   }
@@ -431,6 +433,7 @@ int alegb_destroy(alegb_ctx* ctx) {
   dev_free(ctx->d_clock); dev_free(ctx->d_step_counter);
   for (cudaEvent_t ev : ctx->prof_events) cudaEventDestroy(ev);
   dev_free(ctx->d_Dt); dev_free(ctx->d_LIFTt); dev_free(ctx->d_lam); dev_free(ctx->d_fmask);
+  dev_free(ctx->d_wface); dev_free(ctx->d_force);
   dev_free(ctx->d_Avol); dev_free(ctx->d_Alift); dev_free(ctx->d_AliftP);
   delete ctx;
   return ALEGB_OK;
@@ -642,6 +645,29 @@ int alegb_get_cubature(alegb_ctx* ctx, int* degree, int* Nc, double* rst, double
   if (w) std::memcpy(w, c.w.data(), c.w.size() * sizeof(double));
   if (I) std::memcpy(I, c.I.data(), c.I.size() * sizeof(double));
   if (P) std::memcpy(P, c.P.data(), c.P.size() * sizeof(double));
+  return ALEGB_OK;
+}
+
+int alegb_wall_forces(alegb_ctx* ctx, double t, const double* d_q, int tag, double* h_Fp, double* h_Fv, void* stream) {
+  int rc = check_ready(ctx);
+  if (rc != ALEGB_OK) return rc;
+  if (!d_q || !h_Fp || !h_Fv) return fail(ctx, ALEGB_INVALID_ARG, "NULL pointer");
+  if (tag < 1 || tag > 127) return fail(ctx, ALEGB_INVALID_ARG, "tag must be a boundary tag (1..127)");
+  const int dim = ctx->ref.dim;
+  for (int d = 0; d < dim; ++d) h_Fp[d] = h_Fv[d] = 0.0;
+  if (!ctx->d_EToB) return ALEGB_OK;                    // no tagged faces at all
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  constexpr int kBlocks = 296;
+  if (!ctx->d_force) CU(dev_alloc(ctx, &ctx->d_force, (size_t)(kBlocks + 1) * 6));
+  rc = update_geometry(ctx, t, s);
+  if (rc != ALEGB_OK) return rc;
+  CU(launch_wall_force(dim, ctx->K, ctx->d_EToB, tag, d_q, ctx->d_sgeo, ctx->d_fmask, ctx->d_wface, ctx->ref.Np,
+                       ctx->ref.Nfp, ctx->RT, ctx->d_force, kBlocks, ctx->d_force + (size_t)kBlocks * 6, s));
+  ctx->launches += 2;
+  double out[6];
+  CU(cudaMemcpyAsync(out, ctx->d_force + (size_t)kBlocks * 6, 2 * dim * sizeof(double), cudaMemcpyDeviceToHost, s));
+  CU(cudaStreamSynchronize(s));
+  for (int d = 0; d < dim; ++d) { h_Fp[d] = out[d]; h_Fv[d] = out[dim + d]; }
   return ALEGB_OK;
 }
 

@@ -104,6 +104,10 @@ cudaError_t launch_vertex_motion(int dim, int64_t Nverts, const double* X0, cons
 cudaError_t launch_vertex_rk(int dim, int64_t Nverts, const double* X0, const MotionArgs& m, const double* user_vv,
                              int stage, double t_n, double t_h, double t_e, double dt, const double* ts_dev, double* x_n,
                              double* xv, double* vv, cudaStream_t s);
+// NEXT-3: wall-force integrals; partial[nblocks][2 dim] scratch, out[2 dim] = (F_p, F_v) on the device
+cudaError_t launch_wall_force(int dim, int64_t K, const int8_t* EToB, int tag, const double* q, const double* sgeo,
+                              const int32_t* fmask, const double* wface, int Np, int Nfp, double RT, double* partial,
+                              int nblocks, double* out, cudaStream_t s);
 // clock = {t0, dt, stage times[4]} on the device; _set starts a run of steps, the other advances to the next step
 cudaError_t launch_step_clock(double* clock, long long* counter, cudaStream_t s);
 cudaError_t launch_step_clock_set(double* clock, long long* counter, double t0, double dt, cudaStream_t s);

@@ -331,6 +331,7 @@ bool build_reference(int dim, int N, RefElement& ref, std::string& err) {
   std::vector<qreal> Gf = gram(dim - 1, fex);
   const int ncol = ref.Nfaces * Nfp;
   ref.LIFT.assign(Np * ncol, 0.0);
+  ref.wface.assign(ncol, 0.0);
   for (int f = 0; f < ref.Nfaces; ++f) {
     std::vector<qreal> Vf(Nfp * Nfp);
     for (int i = 0; i < Nfp; ++i) {
@@ -344,6 +345,11 @@ bool build_reference(int dim, int N, RefElement& ref, std::string& err) {
     std::vector<qreal> Vfinv = Vf;
     if (!invert(Vfinv, Nfp)) { err = "singular face Vandermonde"; return false; }
     std::vector<qreal> Mf = matmul(matmul(transpose(Vfinv, Nfp, Nfp), Gf, Nfp, Nfp, Nfp), Vfinv, Nfp, Nfp, Nfp);
+    for (int j = 0; j < Nfp; ++j) {
+      qreal s = 0;
+      for (int i = 0; i < Nfp; ++i) s += Mf[i * Nfp + j];
+      ref.wface[f * Nfp + j] = (double)s;
+    }
     for (int r = 0; r < Np; ++r)
       for (int j = 0; j < Nfp; ++j) {
         qreal s = 0;

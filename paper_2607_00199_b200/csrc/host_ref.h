@@ -16,6 +16,7 @@ struct RefElement {
   std::vector<double> D[3];    // [Np][Np] row-major differentiation matrices D_a = M^-1 S_a
   std::vector<double> LIFT;    // [Np][Nfaces*Nfp]
   std::vector<double> w;       // [Np] 1^T M
+  std::vector<double> wface;   // [Nfaces][Nfp] 1^T M^f on the nodes of each face (face quadrature weights, sum 2)
   std::vector<int> fmask;      // [Nfaces][Nfp]
   int face_verts[4][3];        // local vertex numbers of each face
   int node_of(const int* weights) const;  // lattice tuple -> node index

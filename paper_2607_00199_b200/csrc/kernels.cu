@@ -181,6 +181,95 @@ cudaError_t launch_step_clock_set(double* clock, long long* counter, double t0, 
 }
 
 // ------------------------------------------------------------------------------------------------------------------
+// NEXT-3: pressure and viscous force on the faces tagged `tag` (p = rho RT L53, sigma L51):
+//   F_p = - int p n_b dS,  F_v = int sigma . n_b dS,  n_b = -n^ (outward normal of the body),
+// face integral by the nodal face quadrature sJ sum_m (1^T M^f)_m g_m (reading R22).  One thread per element face,
+// fixed grid and an ordered second pass: the result is deterministic.
+template <int DIM>
+__global__ void wall_force_kernel(int64_t K, const int8_t* __restrict__ EToB, int tag, const double* __restrict__ q,
+                                  const double* __restrict__ sgeo, const int32_t* __restrict__ fmask,
+                                  const double* __restrict__ wface, int Np, int Nfp, double RT,
+                                  double* __restrict__ partial) {
+  constexpr int Nf = DIM == 2 ? 6 : 10, Nfaces = DIM + 1, NO = 2 * DIM;
+  double acc[NO];
+#pragma unroll
+  for (int x = 0; x < NO; ++x) acc[x] = 0.0;
+  const int64_t total = K * Nfaces;
+  for (int64_t ef = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; ef < total; ef += (int64_t)gridDim.x * blockDim.x) {
+    if (EToB[ef] != tag) continue;
+    const int64_t e = ef / Nfaces;
+    const int f = (int)(ef - e * Nfaces);
+    const double* sg = sgeo + ef * (DIM + 2);
+    double nb[DIM];
+#pragma unroll
+    for (int d = 0; d < DIM; ++d) nb[d] = -sg[d];
+    const double sJ = sg[DIM];
+    const double* qe = q + e * Nf * Np;
+    for (int m = 0; m < Nfp; ++m) {
+      const int n = fmask[f * Nfp + m];
+      const double w = sJ * wface[f * Nfp + m];
+      double v[Nf];
+#pragma unroll
+      for (int k = 0; k < Nf; ++k) v[k] = qe[k * Np + n];
+      const double p = RT * v[0], ir = 1.0 / v[0];
+      double sig[DIM][DIM];
+      if constexpr (DIM == 2) {
+        sig[0][1] = sig[1][0] = -RT * (v[3] - v[1] * v[2] * ir);
+        sig[0][0] = -RT * (ALEGB_SQRT2 * v[4] - v[1] * v[1] * ir);
+        sig[1][1] = -RT * (ALEGB_SQRT2 * v[5] - v[2] * v[2] * ir);
+      } else {
+        sig[0][1] = sig[1][0] = -RT * (v[4] - v[1] * v[2] * ir);
+        sig[0][2] = sig[2][0] = -RT * (v[5] - v[1] * v[3] * ir);
+        sig[1][2] = sig[2][1] = -RT * (v[6] - v[2] * v[3] * ir);
+        sig[0][0] = -RT * (ALEGB_SQRT2 * v[7] - v[1] * v[1] * ir);
+        sig[1][1] = -RT * (ALEGB_SQRT2 * v[8] - v[2] * v[2] * ir);
+        sig[2][2] = -RT * (ALEGB_SQRT2 * v[9] - v[3] * v[3] * ir);
+      }
+#pragma unroll
+      for (int i = 0; i < DIM; ++i) {
+        acc[i] -= w * p * nb[i];
+        double s = 0.0;
+#pragma unroll
+        for (int j = 0; j < DIM; ++j) s = fma(sig[i][j], nb[j], s);
+        acc[DIM + i] = fma(w, s, acc[DIM + i]);
+      }
+    }
+  }
+  __shared__ double red[256][NO];
+#pragma unroll
+  for (int x = 0; x < NO; ++x) red[threadIdx.x][x] = acc[x];
+  __syncthreads();
+  for (int s = blockDim.x / 2; s > 0; s >>= 1) {
+    if ((int)threadIdx.x < s) {
+#pragma unroll
+      for (int x = 0; x < NO; ++x) red[threadIdx.x][x] += red[threadIdx.x + s][x];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int x = 0; x < NO; ++x) partial[blockIdx.x * NO + x] = red[0][x];
+  }
+}
+
+__global__ void wall_force_reduce_kernel(const double* __restrict__ partial, int nblocks, int NO, double* __restrict__ out) {
+  const int x = threadIdx.x;
+  if (x >= NO) return;
+  double s = 0.0;
+  for (int b = 0; b < nblocks; ++b) s += partial[b * NO + x];
+  out[x] = s;
+}
+
+cudaError_t launch_wall_force(int dim, int64_t K, const int8_t* EToB, int tag, const double* q, const double* sgeo,
+                              const int32_t* fmask, const double* wface, int Np, int Nfp, double RT, double* partial,
+                              int nblocks, double* out, cudaStream_t s) {
+  if (dim == 2) wall_force_kernel<2><<<nblocks, 256, 0, s>>>(K, EToB, tag, q, sgeo, fmask, wface, Np, Nfp, RT, partial);
+  else wall_force_kernel<3><<<nblocks, 256, 0, s>>>(K, EToB, tag, q, sgeo, fmask, wface, Np, Nfp, RT, partial);
+  wall_force_reduce_kernel<<<1, 32, 0, s>>>(partial, nblocks, 2 * dim, out);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------------
 // a2: geometric factors.  One thread per element, registers only (as PAPER.md:L193).
 template <int DIM>
 __global__ void geometry_kernel(int64_t K, const int32_t* __restrict__ EToV, const double* __restrict__ xv,

@@ -1,6 +1,8 @@
 """Shared test helpers: build an oracle Problem (and, on the GPU side, a library context) from a workload dict."""
 import numpy as np
 
+from workloads import configs, meshes
+
 
 def oracle_problem(cfg, ref):
     from oracle.rhs import Problem
@@ -41,3 +43,15 @@ def submesh(cfg, EToE, samples, rings):
     sub["q0"] = np.ascontiguousarray(cfg["q0"][patch])
     where = np.searchsorted(patch, samples)
     return sub, patch, where
+
+
+def swimmer_small(lam, n=(12, 6, 6), lo=(-4.0, -3.0, -3.0), hi=(8.0, 3.0, 3.0)):
+    """config 5 shape with a body fat enough to be resolved by a coarse grid (wall faces, far field, PML)."""
+    cfg = configs.config5(lam, nx=n[0], ny=n[1], nz=n[2])
+    X0, EToV, EToB, sigma = meshes.swimmer_box(n[0], n[1], n[2], half_height=1.2, half_width=1.2,
+                                               lo=lo, hi=hi)
+    cfg.update(X0=X0, EToV=EToV, EToB=EToB, pml_sigma=sigma)
+    cfg["motion_params"] = cfg["motion_params"].copy()
+    cfg["motion_params"][5] = 2.0                   # R_rigid: make the layer around the body move
+    cfg["dt"] = configs.cfl_dt(3, 3, X0, EToV, cfg["RT"], 0.5, 0.2 * cfg["motion_params"][4])
+    return configs._finish(cfg, lam)

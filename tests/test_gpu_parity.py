@@ -13,7 +13,7 @@ from oracle import mesh as omesh
 from oracle import motion as omotion
 from oracle import physics, sark
 from workloads import configs, meshes
-from helpers import oracle_problem, rel_linf, submesh
+from helpers import oracle_problem, rel_linf, submesh, swimmer_small
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -37,18 +37,6 @@ def perturbed(cfg, amp=1e-3, seed=7):
     """Initial state with seeded element-wise noise, so that every face carries a jump."""
     rng = np.random.default_rng(seed)
     return cfg["q0"] * (1.0 + amp * rng.standard_normal(cfg["q0"].shape))
-
-
-def swimmer_small(lam, n=(12, 6, 6), lo=(-4.0, -3.0, -3.0), hi=(8.0, 3.0, 3.0)):
-    """config 5 shape with a body fat enough to be resolved by a coarse grid (wall faces, far field, PML)."""
-    cfg = configs.config5(lam, nx=n[0], ny=n[1], nz=n[2])
-    X0, EToV, EToB, sigma = meshes.swimmer_box(n[0], n[1], n[2], half_height=1.2, half_width=1.2,
-                                               lo=lo, hi=hi)
-    cfg.update(X0=X0, EToV=EToV, EToB=EToB, pml_sigma=sigma)
-    cfg["motion_params"] = cfg["motion_params"].copy()
-    cfg["motion_params"][5] = 2.0                   # R_rigid: make the layer around the body move
-    cfg["dt"] = configs.cfl_dt(3, 3, X0, EToV, cfg["RT"], 0.5, 0.2 * cfg["motion_params"][4])
-    return configs._finish(cfg, lam)
 
 
 def make_case(name, refs):
@@ -563,4 +551,32 @@ def test_cubature_free_stream_on_gpu(refs, B):
     ctx.alegb_step(dq, 0.0, cfg["dt"], 50)
     torch.cuda.synchronize()
     assert np.abs(dq.cpu().numpy() - cfg["q0"]).max() < 1e-13
+    ctx.close()
+
+
+# ------------------------------------------------------------------ NEXT-3: wall-force integrals (L308, L369)
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", ["cfg3", "cfg5", "cfg1"])
+def test_wall_forces_match_oracle(name, refs, B):
+    from oracle import forces
+    ref, cfg = make_case(name, refs)
+    P = oracle_problem(cfg, ref)
+    q = perturbed(cfg, amp=2e-2)
+    ctx = B.context_from_config(cfg)
+    for t in (0.0, 0.4):
+        Fp, Fv = ctx.alegb_wall_forces(t, dev(q), 1)
+        Fp2, Fv2 = ctx.alegb_wall_forces(t, dev(q), 1)
+        assert np.array_equal(Fp, Fp2) and np.array_equal(Fv, Fv2)          # deterministic
+        op, ov = forces.wall_force(P, q, t)
+        scale = max(np.abs(op).max(), np.abs(ov).max(), 1e-300)
+        if name == "cfg1":                                                  # no wall faces
+            assert not Fp.any() and not Fv.any() and not op.any()
+        else:
+            # absolute scale of the summed terms: the integral of |p| over the wall
+            g = P.geometry(t)
+            area = sum(2.0 * g["sJ"][P.EToB[:, f] == 1, f].sum() for f in range(ref.Nfaces))
+            assert area > 0
+            assert np.abs(Fp - op).max() <= 1e-12 * area * cfg["RT"] * np.abs(q[:, 0]).max()
+            assert np.abs(Fv - ov).max() <= 1e-12 * area * cfg["RT"] * np.abs(q).max()
+            assert scale > 0
     ctx.close()
