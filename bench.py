@@ -78,7 +78,7 @@ class ClockSampler:
         self.proc = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.FIELDS,
-                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.tmp,
+                                          "--format=csv,noheader,nounits", "-lms", "20"], stdout=self.tmp,
                                          stderr=subprocess.DEVNULL)
         except Exception:
             self.proc = None
