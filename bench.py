@@ -194,6 +194,7 @@ def main():
                     help="nonlinear relaxation: collocated (default, DESIGN.md R8) or cubature-projected (NEXT-1)")
     ap.add_argument("--coords", default="closed", choices=["closed", "rk"],
                     help="vertex positions: closed-form law (default, R9) or advanced by the solver's RK4 (NEXT-2)")
+    ap.add_argument("--no-overlap", action="store_true", help="a1/a2 of the next stage in order instead of beside the stage kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -222,6 +223,8 @@ def main():
     cfg = make_config(args.config, lam)
     ctx = B.context_from_config(cfg, local_rank)
     ctx.alegb_set_kernel(args.kernel)
+    if args.no_overlap:
+        ctx.alegb_set_geometry_overlap(False)
     if args.relax == "cubature":
         ctx.alegb_set_relaxation(B.RELAX_CUBATURE)
     if args.coords == "rk":

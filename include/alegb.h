@@ -192,6 +192,11 @@ int64_t alegb_launch_count(const alegb_ctx* ctx);
  * (producer/consumer warps), 3 = warp-per-4-elements DMMA kernel; 2 and 3 return ALEGB_UNSUPPORTED if there is none.
  * All compute the same operator; tests run all of them. */
 int alegb_set_kernel(alegb_ctx* ctx, int kind);
+/* Inside a step the vertex-motion and geometric-factor kernels (a1, a2) of stage i+1 depend on time only; with the
+ * overlap on (default) they run on a stream of the library's own beside the stage kernel of stage i, into a second
+ * set of geometry arrays, joined by events (captured into the step graph as a parallel branch).  Same kernels, same
+ * results bit for bit; off = everything in order on the caller's stream. */
+int alegb_set_geometry_overlap(alegb_ctx* ctx, int on);
 /* alegb_step with nsteps >= 2 replays ONE captured CUDA graph per step (clock kernel + the a1, a2, a3-a8 launches of
  * the four stages; stage times t_n + c_i dt are computed on the device with the host loop's IEEE operations, so the
  * result is bit-identical to nsteps single-step calls).  It removes the per-launch host cost that bounds the small

@@ -34,6 +34,7 @@ _SIGNATURES = {
     "alegb_set_motion_user": (_c.c_int, [_P, _P, _P]),
     "alegb_set_coordinate_mode": (_c.c_int, [_P, _c.c_int, _c.c_double]),
     "alegb_set_relaxation": (_c.c_int, [_P, _c.c_int]),
+    "alegb_set_geometry_overlap": (_c.c_int, [_P, _c.c_int]),
     "alegb_wall_forces": (_c.c_int, [_P, _c.c_double, _P, _c.c_int, _P, _P, _P]),
     "alegb_get_cubature": (_c.c_int, [_P, _c.POINTER(_c.c_int), _c.POINTER(_c.c_int), _P, _P, _P, _P]),
     "alegb_get_positions": (_c.c_int, [_P, _P, _P]),
@@ -152,6 +153,9 @@ class Context:
         Fp, Fv = np.zeros(self.dim), np.zeros(self.dim)
         self._check(_lib.alegb_wall_forces(self._h, float(t), _dev(d_q), int(tag), Fp.ctypes.data, Fv.ctypes.data, _stream(stream)))
         return Fp, Fv
+
+    def alegb_set_geometry_overlap(self, on):
+        self._check(_lib.alegb_set_geometry_overlap(self._h, int(bool(on))))
 
     def alegb_set_relaxation(self, mode):
         self._check(_lib.alegb_set_relaxation(self._h, int(mode)))

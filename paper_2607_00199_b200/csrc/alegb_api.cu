@@ -43,6 +43,16 @@ struct alegb_ctx {
   int32_t *d_EToV = nullptr, *d_vmapP = nullptr;
   int8_t* d_EToB = nullptr;
   double *d_vgeo = nullptr, *d_sgeo = nullptr, *d_vvel = nullptr;
+  // second set of geometry arrays + side stream: a1/a2 of stage i+1 depend on time only, so inside a step they run
+  // beside the stage kernel of stage i (the persistent stage kernel leaves threads and registers for them)
+  double *d_vgeo1 = nullptr, *d_sgeo1 = nullptr, *d_vvel1 = nullptr;
+  int geo_buf = 0;                       // which set update_geometry / fill_common use
+  bool overlap_geometry = true;
+  cudaStream_t geo_stream = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_geo[4] = {nullptr, nullptr, nullptr, nullptr}, ev_stage[4] = {nullptr, nullptr, nullptr, nullptr};
+  double* vg() const { return geo_buf ? d_vgeo1 : d_vgeo; }
+  double* sg() const { return geo_buf ? d_sgeo1 : d_sgeo; }
+  double* vvl() const { return geo_buf ? d_vvel1 : d_vvel; }
   int32_t *d_pml_index = nullptr, *d_pml_elems = nullptr;
   double* d_pml_sigma = nullptr;
   // device: step workspace
@@ -104,6 +114,7 @@ void free_mesh(alegb_ctx* ctx) {
   dev_free(ctx->d_R); ctx->relax_mode = ALEGB_RELAX_COLLOCATION;
   dev_free(ctx->d_X0); dev_free(ctx->d_xv); dev_free(ctx->d_vv); dev_free(ctx->d_EToV); dev_free(ctx->d_vmapP);
   dev_free(ctx->d_EToB); dev_free(ctx->d_vgeo); dev_free(ctx->d_sgeo); dev_free(ctx->d_vvel);
+  dev_free(ctx->d_vgeo1); dev_free(ctx->d_sgeo1); dev_free(ctx->d_vvel1); ctx->geo_buf = 0;
   dev_free(ctx->d_pml_index); dev_free(ctx->d_pml_elems); dev_free(ctx->d_pml_sigma);
   dev_free(ctx->d_Q1); dev_free(ctx->d_Q2); dev_free(ctx->d_F0); dev_free(ctx->d_ACC); dev_free(ctx->d_Qhost);
   dev_free(ctx->d_AUX); dev_free(ctx->d_AUXS); dev_free(ctx->d_AUXACC);
@@ -121,7 +132,7 @@ int update_geometry(alegb_ctx* ctx, double t, cudaStream_t s, const double* t_de
     CU(launch_vertex_motion(dim, ctx->Nverts, ctx->d_X0, ctx->motion, t, t_dev, ctx->d_xv, ctx->d_vv, s));
     ctx->launches++;
   }
-  CU(launch_geometry(dim, ctx->K, ctx->d_EToV, ctx->d_xv, ctx->d_vv, ctx->d_vgeo, ctx->d_sgeo, ctx->d_vvel, s));
+  CU(launch_geometry(dim, ctx->K, ctx->d_EToV, ctx->d_xv, ctx->d_vv, ctx->vg(), ctx->sg(), ctx->vvl(), s));
   ctx->launches++;
   return ALEGB_OK;
 }
@@ -135,7 +146,7 @@ int update_geometry_rk(alegb_ctx* ctx, int stage, double t0, double dt, cudaStre
                       ctx->d_xn, ctx->d_xv, ctx->d_vv, s));
   ctx->launches++;
   if (stage < 4) {
-    CU(launch_geometry(dim, ctx->K, ctx->d_EToV, ctx->d_xv, ctx->d_vv, ctx->d_vgeo, ctx->d_sgeo, ctx->d_vvel, s));
+    CU(launch_geometry(dim, ctx->K, ctx->d_EToV, ctx->d_xv, ctx->d_vv, ctx->vg(), ctx->sg(), ctx->vvl(), s));
     ctx->launches++;
   }
   return ALEGB_OK;
@@ -144,7 +155,7 @@ int update_geometry_rk(alegb_ctx* ctx, int stage, double t0, double dt, cudaStre
 void fill_common(const alegb_ctx* ctx, StageArgs& a) {
   std::memset(&a, 0, sizeof(a));
   a.K = ctx->K;
-  a.vgeo = ctx->d_vgeo; a.sgeo = ctx->d_sgeo; a.vvel = ctx->d_vvel;
+  a.vgeo = ctx->vg(); a.sgeo = ctx->sg(); a.vvel = ctx->vvl();
   a.vmapP = ctx->d_vmapP; a.EToB = ctx->d_EToB;
   a.pml_index = ctx->d_pml_index; a.pml_sigma = ctx->d_pml_sigma;
   a.Dt_ops = ctx->d_Dt; a.LIFTt = ctx->d_LIFTt; a.lam = ctx->d_lam; a.fmask = ctx->d_fmask;
@@ -155,7 +166,7 @@ void fill_common(const alegb_ctx* ctx, StageArgs& a) {
 void fill_common(const alegb_ctx* ctx, PmlArgs& a) {
   std::memset(&a, 0, sizeof(a));
   a.Kpml = ctx->Kpml; a.pml_elems = ctx->d_pml_elems; a.pml_sigma = ctx->d_pml_sigma;
-  a.vgeo = ctx->d_vgeo; a.sgeo = ctx->d_sgeo; a.vvel = ctx->d_vvel;
+  a.vgeo = ctx->vg(); a.sgeo = ctx->sg(); a.vvel = ctx->vvl();
   a.vmapP = ctx->d_vmapP; a.EToB = ctx->d_EToB;
   a.Dt_ops = ctx->d_Dt; a.LIFTt = ctx->d_LIFTt; a.lam = ctx->d_lam; a.fmask = ctx->d_fmask;
   a.Avol = ctx->d_Avol; a.AliftP = ctx->d_AliftP;
@@ -235,11 +246,46 @@ int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t
   auto B = [&](int k, int j) { return stiff[k] ? bs[j] : b0[j]; };
   const double cstage[4] = {0.0, 0.5, 0.5, 1.0};
   const bool pml = ctx->Kpml > 0;
+  const bool overlap = ctx->overlap_geometry;
+  if (overlap && !ctx->geo_stream) {
+    CU(cudaStreamCreateWithFlags(&ctx->geo_stream, cudaStreamNonBlocking));
+    CU(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
+    for (int i = 0; i < 4; ++i) {
+      CU(cudaEventCreateWithFlags(&ctx->ev_geo[i], cudaEventDisableTiming));
+      CU(cudaEventCreateWithFlags(&ctx->ev_stage[i], cudaEventDisableTiming));
+    }
+  }
   for (int i = 0; i < 4; ++i) {
     const double ti = t0 + cstage[i] * dt;
-    int rc = ctx->coord_mode == ALEGB_COORDS_RK ? update_geometry_rk(ctx, i, t0, dt, s, t_dev)
-                                                 : update_geometry(ctx, ti, s, t_dev ? t_dev + i : nullptr);
+    // a1 + a2 of stage `j` into geometry set j & 1, on stream `gs`
+    auto geometry_of = [&](int j, cudaStream_t gs) {
+      ctx->geo_buf = j & 1;
+      const double tj = t0 + cstage[j] * dt;
+      return ctx->coord_mode == ALEGB_COORDS_RK ? update_geometry_rk(ctx, j, t0, dt, gs, t_dev)
+                                                 : update_geometry(ctx, tj, gs, t_dev ? t_dev + j : nullptr);
+    };
+    (void)ti;
+    int rc = ALEGB_OK;
+    if (i == 0) {
+      rc = geometry_of(0, s);
+      if (rc == ALEGB_OK && overlap) {      // fork: the side stream starts after stage 0's geometry
+        CU(cudaEventRecord(ctx->ev_fork, s));
+        CU(cudaStreamWaitEvent(ctx->geo_stream, ctx->ev_fork, 0));
+      }
+    } else if (overlap) {
+      CU(cudaStreamWaitEvent(s, ctx->ev_geo[i], 0));
+    } else {
+      rc = geometry_of(i, s);
+    }
     if (rc != ALEGB_OK) return rc;
+    if (overlap && i < 3) {
+      // stage i+1's geometry beside stage i's kernels; its arrays were last read by stage i-1
+      if (i >= 1) CU(cudaStreamWaitEvent(ctx->geo_stream, ctx->ev_stage[i - 1], 0));
+      rc = geometry_of(i + 1, ctx->geo_stream);
+      if (rc != ALEGB_OK) return rc;
+      CU(cudaEventRecord(ctx->ev_geo[i + 1], ctx->geo_stream));
+    }
+    ctx->geo_buf = i & 1;
     StageArgs a;
     fill_common(ctx, a);
     a.q_in = i == 0 ? q_n : outs[i - 1];
@@ -286,7 +332,9 @@ int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t
       CU(launch_pml_any(ctx, p, s));
       ctx->launches++;
     }
+    if (overlap) CU(cudaEventRecord(ctx->ev_stage[i], s));
   }
+  ctx->geo_buf = 0;
   if (ctx->coord_mode == ALEGB_COORDS_RK && advance_coords) return update_geometry_rk(ctx, 4, t0, dt, s, t_dev);
   return ALEGB_OK;
 }
@@ -430,6 +478,12 @@ int alegb_destroy(alegb_ctx* ctx) {
   free_mesh(ctx);
   drop_step_graph(ctx);
   if (ctx->capture_stream) cudaStreamDestroy(ctx->capture_stream);
+  if (ctx->geo_stream) cudaStreamDestroy(ctx->geo_stream);
+  if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+  for (int i = 0; i < 4; ++i) {
+    if (ctx->ev_geo[i]) cudaEventDestroy(ctx->ev_geo[i]);
+    if (ctx->ev_stage[i]) cudaEventDestroy(ctx->ev_stage[i]);
+  }
   dev_free(ctx->d_clock); dev_free(ctx->d_step_counter);
   for (cudaEvent_t ev : ctx->prof_events) cudaEventDestroy(ev);
   dev_free(ctx->d_Dt); dev_free(ctx->d_LIFTt); dev_free(ctx->d_lam); dev_free(ctx->d_fmask);
@@ -505,6 +559,9 @@ int alegb_mesh_upload(alegb_ctx* ctx, int64_t Nverts, const double* X0, int64_t 
   CU(dev_alloc(ctx, &ctx->d_vgeo, (size_t)K * (dim * dim + 1)));
   CU(dev_alloc(ctx, &ctx->d_sgeo, (size_t)K * nv * (dim + 2)));
   CU(dev_alloc(ctx, &ctx->d_vvel, (size_t)K * nv * dim));
+  CU(dev_alloc(ctx, &ctx->d_vgeo1, (size_t)K * (dim * dim + 1)));
+  CU(dev_alloc(ctx, &ctx->d_sgeo1, (size_t)K * nv * (dim + 2)));
+  CU(dev_alloc(ctx, &ctx->d_vvel1, (size_t)K * nv * dim));
   CU(dev_alloc(ctx, &ctx->d_Q1, state));
   CU(dev_alloc(ctx, &ctx->d_Q2, state));
   CU(dev_alloc(ctx, &ctx->d_F0, state));
@@ -885,6 +942,13 @@ int alegb_set_kernel(alegb_ctx* ctx, int kind) {
   if (kind == 2 && !ctx->pipe_ok) return fail(ctx, ALEGB_UNSUPPORTED, "no pipelined DMMA stage kernel for this (dim, N)");
   if (kind == 3 && !ctx->mma_ok) return fail(ctx, ALEGB_UNSUPPORTED, "no DMMA stage kernel for this (dim, N)");
   ctx->kernel_mode = kind;
+  ctx->config_version++;
+  return ALEGB_OK;
+}
+
+int alegb_set_geometry_overlap(alegb_ctx* ctx, int on) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  ctx->overlap_geometry = on != 0;
   ctx->config_version++;
   return ALEGB_OK;
 }

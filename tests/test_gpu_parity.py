@@ -580,3 +580,28 @@ def test_wall_forces_match_oracle(name, refs, B):
             assert np.abs(Fv - ov).max() <= 1e-12 * area * cfg["RT"] * np.abs(q).max()
             assert scale > 0
     ctx.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", ["cfg1", "cfg3", "cfg4"])
+def test_geometry_overlap_is_bit_identical(name, refs, B):
+    """a1/a2 of stage i+1 beside the stage kernel of stage i (side stream, second geometry set): same bits as in-order
+    launches, through the graph and through direct launches, closed-form and RK coordinates."""
+    ref, cfg = make_case(name, refs)
+    q = perturbed(cfg)
+    outs = []
+    for overlap, graph, rk in ((1, 1, 0), (0, 1, 0), (1, 0, 0), (0, 0, 0), (1, 1, 1), (0, 0, 1)):
+        ctx = B.context_from_config(cfg)
+        ctx.alegb_set_geometry_overlap(overlap)
+        ctx.alegb_set_graph(graph)
+        if rk:
+            ctx.alegb_set_coordinate_mode(B.COORDS_RK, 0.0)
+        dq = dev(q)
+        ctx.alegb_step(dq, 0.0, cfg["dt"], 7)
+        ctx.alegb_step(dq, 7 * cfg["dt"], cfg["dt"], 1)
+        torch.cuda.synchronize()
+        outs.append(dq.cpu().numpy())
+        ctx.close()
+    for o in outs[1:4]:
+        assert np.array_equal(outs[0], o)
+    assert np.array_equal(outs[4], outs[5])
