@@ -364,8 +364,10 @@ def test_graph_replay_is_bit_identical_to_direct_launches(name, refs, B):
     ctx.close()
 
 
-def test_full_size_throughput_config_sampled(refs, B):
-    """BASELINE.json configs[3] at full size (196,608 tets, N = 4), the launch configuration bench.py times.
+@pytest.mark.parametrize("relax", ["collocation", "cubature"])
+def test_full_size_throughput_config_sampled(relax, refs, B):
+    """BASELINE.json configs[3] at full size (196,608 tets, N = 4), the launch configuration bench.py times
+    (default mode, and bench.py --relax cubature).
     The oracle computes a sample of elements one patch at a time (helpers.submesh): F needs the face neighbours,
     stage state i needs i rings of them."""
     ref = refs(3, 4)
@@ -373,6 +375,9 @@ def test_full_size_throughput_config_sampled(refs, B):
     assert cfg["K"] == 196608
     conn = omesh.connect(ref, cfg["EToV"], cfg["vertex_equiv"])
     ctx = B.context_from_config(cfg)
+    cfg["relax"] = relax
+    if relax == "cubature":
+        ctx.alegb_set_relaxation(B.RELAX_CUBATURE)
     q = perturbed(cfg, amp=1e-4)
     cfg["q0"] = q
     dq = dev(q)
