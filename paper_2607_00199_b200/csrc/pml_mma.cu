@@ -233,15 +233,31 @@ __global__ void __launch_bounds__(pmlmma::Cfg<DIM, N>::Threads, 1) pml_mma_kerne
         // RK inputs of this direction, requested before the LIFT contraction so that their latency hides behind it
         const double sig = evalid ? a.pml_sigma[p * DIM + dd] : 0.0;
         const int64_t base = ((p * DIM + dd) * Nf) * Np + nn;
+        // (p and nn are clamped, so the addresses are valid for every lane: straight-line loads behind one uniform
+        //  branch per array -- per-lane predicates made the compiler wait for each load before issuing the next,
+        //  53 % of the kernel's stall samples, profiles/r1_pml_kernel.md)
         double xi[Nf], xn[Nf], xa[Nf];
+        {
+          const double* pi = a.aux_in + base;
 #pragma unroll
-        for (int k = 0; k < Nf; ++k) {
-          xi[k] = xn[k] = xa[k] = 0.0;
-          if (evalid) {
-            xi[k] = a.aux_in[base + k * Np];
-            if (a.aux_n) xn[k] = a.aux_n == a.aux_in ? xi[k] : a.aux_n[base + k * Np];
-            if (a.acc_in) xa[k] = a.acc_in[base + k * Np];
+          for (int k = 0; k < Nf; ++k) xi[k] = pi[k * Np];
+        }
+#pragma unroll
+        for (int k = 0; k < Nf; ++k) { xn[k] = 0.0; xa[k] = 0.0; }
+        if (a.aux_n != nullptr) {
+          if (a.aux_n == a.aux_in) {
+#pragma unroll
+            for (int k = 0; k < Nf; ++k) xn[k] = xi[k];
+          } else {
+            const double* pn = a.aux_n + base;
+#pragma unroll
+            for (int k = 0; k < Nf; ++k) xn[k] = pn[k * Np];
           }
+        }
+        if (a.acc_in != nullptr) {
+          const double* pa = a.acc_in + base;
+#pragma unroll
+          for (int k = 0; k < Nf; ++k) xa[k] = pa[k * Np];
         }
         // surface part: LIFT of the direction's flux tile, accumulated into the same registers
         const double* gd = gt + dd * C::gtile_doubles;
