@@ -59,6 +59,10 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
 __device__ __forceinline__ void prefetch_l2(const void* p, uint32_t bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void cp_async8(double* dst, const double* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 __device__ __forceinline__ void team_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
@@ -122,19 +126,46 @@ __global__ void __launch_bounds__(pmlmma::Cfg<DIM, N>::Threads, 1) pml_mma_kerne
         }
       }
     }
-    // ---- q tile of the quad's elements, rows (element, field), node stride S; missing elements read as zero
-    for (int x = tl; x < EG * Nf * Np; x += TT) {
+    // ---- element ids of the quad (one load per element, shared by everything below)
+    int eid[EG];
+#pragma unroll
+    for (int el = 0; el < EG; ++el) eid[el] = a.pml_elems[p0 + (el < nel ? el : 0)];
+    // ---- q tile of the quad's elements, rows (element, field), node stride S, asynchronously (rows of missing
+    //      elements keep the previous quad's finite values; nothing of them is stored)
+    for (int x = tl; x < nel * Nf * Np; x += TT) {
       const int row = x / Np, j = x - row * Np;
       const int el = row / Nf, k = row - el * Nf;
-      double v = 0.0;
-      if (el < nel) v = a.q_in[((int64_t)a.pml_elems[p0 + el] * Nf + k) * Np + j];
-      qt[row * S + j] = v;
+      int e = eid[0];
+#pragma unroll
+      for (int u = 1; u < EG; ++u) if (el == u) e = eid[u];
+      cp_async8(qt + row * S + j, a.q_in + ((int64_t)e * Nf + k) * Np + j);
     }
+    // ---- indices of my face nodes (boundary tag, exterior node), requested together before the tile is waited for
+    constexpr int FR = (EG * NFN + TT - 1) / TT;
+    int f_tag[FR], f_idP[FR], f_e[FR];
+#pragma unroll
+    for (int r = 0; r < FR; ++r) {
+      const int x = tl + r * TT;
+      f_tag[r] = 0; f_idP[r] = 0; f_e[r] = eid[0];
+      if (x < nel * NFN) {
+        const int fe = x / NFN, m = x - fe * NFN;
+        int e = eid[0];
+#pragma unroll
+        for (int u = 1; u < EG; ++u) if (fe == u) e = eid[u];
+        f_e[r] = e;
+        if (a.EToB) f_tag[r] = a.EToB[(int64_t)e * Nfaces + m / Nfp];
+        f_idP[r] = a.vmapP[(int64_t)e * NFN + m];
+      }
+    }
+    cp_async_wait_all();
     team_sync(1 + team, TT);
     // ---- directional flux tiles: one gather of q+, one |A_n|[q], DIM directional pieces per face node
-    for (int x = tl; x < nel * NFN; x += TT) {
+#pragma unroll
+    for (int r = 0; r < FR; ++r) {
+      const int x = tl + r * TT;
+      if (x >= nel * NFN) continue;
       const int fe = x / NFN, m = x - fe * NFN;
-      const int64_t ee = a.pml_elems[p0 + fe];
+      const int64_t ee = f_e[r];
       const int f = m / Nfp, n = sfmask[m];
       double qM[Nf], qP[Nf];
 #pragma unroll
@@ -144,9 +175,9 @@ __global__ void __launch_bounds__(pmlmma::Cfg<DIM, N>::Threads, 1) pml_mma_kerne
 #pragma unroll
       for (int d = 0; d < DIM; ++d) nh[d] = sg[d];
       const double Fscale = sg[DIM + 1];
-      const int tag = a.EToB ? a.EToB[ee * Nfaces + f] : 0;
+      const int tag = f_tag[r];
       if (tag == 0) {
-        const int idP = a.vmapP[ee * NFN + m];
+        const int idP = f_idP[r];
         const int eP = idP / Np, nP = idP - eP * Np;
         const double* qp = a.q_in + (int64_t)eP * Nf * Np + nP;
 #pragma unroll
@@ -207,7 +238,9 @@ __global__ void __launch_bounds__(pmlmma::Cfg<DIM, N>::Threads, 1) pml_mma_kerne
       const int nn = n < Np ? n : Np - 1;
       const bool evalid = c < nel && n < Np;
       const int64_t p = p0 + (c < nel ? c : 0);
-      const int64_t e = a.pml_elems[p];
+      int64_t e = eid[0];
+#pragma unroll
+      for (int u = 1; u < EG; ++u) if (c == u && c < nel) e = eid[u];
       double G[DIM * DIM];
       {
         const double* vg = a.vgeo + e * (DIM * DIM + 1);
