@@ -147,6 +147,13 @@ def test_argument_validation():
     with pytest.raises(B.AlegbError):
         ctx.alegb_set_motion(17, [])
     ctx.alegb_set_motion(B.MOTION_SINES_PRODUCT, [0.1, 1.0, 1.0, 1.0, 0.0, 0.0])
+    for call in (lambda: ctx.alegb_set_relaxation(7), lambda: ctx.alegb_set_coordinate_mode(-1, 0.0)):
+        with pytest.raises(B.AlegbError) as e:
+            call()
+        assert e.value.status == B.INVALID_ARG
+    ctx.alegb_set_relaxation(B.RELAX_COLLOCATION)        # the default modes need no device
+    ctx.alegb_set_coordinate_mode(B.COORDS_CLOSED_FORM, 0.0)
+    ctx.alegb_set_geometry_overlap(False)
     ctx.close()
 
 
@@ -158,7 +165,10 @@ def test_no_cpu_fallback():
     ctx.alegb_set_params(1.0, 1e-3)
     for call in (lambda: ctx.alegb_rhs(0.0, 16, 16, stream=0), lambda: ctx.alegb_step(16, 0.0, 1e-3, 1, stream=0),
                  lambda: ctx.alegb_geometry(0.0, stream=0), lambda: ctx.alegb_step_host(np.zeros(8), 0.0, 1e-3, 1),
-                 lambda: ctx.alegb_profile_read()):
+                 lambda: ctx.alegb_profile_read(),
+                 # the optional modes and the diagnostics have no host path either
+                 lambda: ctx.alegb_set_relaxation(B.RELAX_CUBATURE), lambda: ctx.alegb_set_coordinate_mode(B.COORDS_RK, 0.0),
+                 lambda: ctx.alegb_get_positions(16, stream=0), lambda: ctx.alegb_wall_forces(0.0, 16, 1, stream=0)):
         with pytest.raises(B.AlegbError) as e:
             call()
         assert e.value.status == B.CUDA_ERROR
