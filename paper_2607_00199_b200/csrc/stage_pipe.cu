@@ -163,7 +163,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
   if (tid == 0) {
     for (int s = 0; s < NS; ++s) {
       mbar_init(&full[s], PT);
-      mbar_init(&empty[s], NB * 32);
+      mbar_init(&empty[s], C::CW * 32);   // every consumer warp takes part in every hand-over (see the consumers)
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -315,8 +315,24 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
     const bool qn_in_tile = a.q_n == a.q_in;
     const bool want_update = a.q_out != nullptr || a.acc_out != nullptr;
     const int nitems = nq_cta * NB;
+    // mbarrier waits test a phase PARITY, so a waiter must never be two phases away from the barrier.  A warp has
+    // an item only in some quads (items cw, cw + CW, ...; NB <= CW items per quad); were it to skip the others, it
+    // could reach a slot whose previous use is not even full yet -- the parity test then passes and it reads stale
+    // data -- or fall two uses behind and wait forever (seen as a hang with two producer groups and a ring of 4, and
+    // reproduced for 3-D N = 1 in a scheduling simulation).  So every consumer warp takes part in the hand-over of
+    // EVERY quad, in order: it waits for `full`, works if it has an item there, and arrives on `empty`.
+    static_assert(NB <= C::CW, "at most one item per quad and consumer warp");
+    int next_q = 0;   // first quad this warp has not yet taken part in
+    auto pass_quads = [&](int upto) {
+      for (; next_q < upto; ++next_q) {
+        mbar_wait(&full[next_q % NS], (next_q / NS) & 1);
+        mbar_arrive(&empty[next_q % NS]);
+      }
+    };
     for (int it = cw; it < nitems; it += C::CW) {
       const int ql = it / NB, nb = it - ql * NB;
+      pass_quads(ql);
+      next_q = ql + 1;
       const int64_t quad = (int64_t)ql * gridDim.x + blockIdx.x;
       const int64_t e0 = quad * EG;
       const int nel = (a.K - e0) < EG ? (int)(a.K - e0) : EG;
@@ -468,6 +484,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
         if (a.acc_out != nullptr) combine(a.coef.ca_n, a.coef.ca_f0, a.coef.ca_acc, a.coef.ca_f, a.acc_out + base);
       }
     }
+    pass_quads(nq_cta);
   }
 }
 

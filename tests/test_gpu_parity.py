@@ -610,3 +610,38 @@ def test_geometry_overlap_is_bit_identical(name, refs, B):
     for o in outs[1:4]:
         assert np.array_equal(outs[0], o)
     assert np.array_equal(outs[4], outs[5])
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("dim,N,n", [(3, 1, 12), (3, 2, 10), (3, 3, 10), (2, 1, 72), (2, 2, 64), (2, 3, 56)])
+def test_low_orders_with_many_quads_per_cta(dim, N, n, refs, B):
+    """Low orders have few work items per quad (NB = 1 at N = 1), so a consumer warp of the pipelined kernel owns an
+    item only in every CW-th quad; with many quads per CTA this is the regime in which a warp that skipped the
+    hand-over of the quads in between could pass an mbarrier parity wait two phases early (stale tile) or hang.
+    Meshes large enough for >= 10 quads per CTA, all three kernels against the oracle."""
+    ref = refs(dim, N)
+    cfg = configs.config4(ref.lam, n=n) if dim == 3 else configs.config2(ref.lam, n=n)
+    cfg["N"] = N
+    cfg = configs._finish(cfg, ref.lam)
+    assert cfg["K"] >= 148 * 4 * 10
+    P = oracle_problem(cfg, ref)
+    q = perturbed(cfg)
+    F, Fabs = P.rhs(q, 0.2, want_abs=True)
+    so, _ = sark.step_debug(P, q, 0.2, cfg["dt"])
+    for kernel in KERNELS:
+        ctx = B.context_from_config(cfg)
+        try:
+            ctx.alegb_set_kernel(kernel)
+        except B.AlegbError:
+            ctx.close()
+            continue
+        dq, dF = dev(q), torch.empty(q.shape, dtype=torch.float64, device="cuda")
+        st = torch.empty((4,) + q.shape, dtype=torch.float64, device="cuda")
+        for rep in range(3):                                  # timing-dependent failures: a few repetitions
+            ctx.alegb_rhs(0.2, dq, dF)
+            ctx.alegb_step_debug(dq, 0.2, cfg["dt"], st)
+            torch.cuda.synchronize()
+            assert (np.abs(dF.cpu().numpy() - F) <= TOL_F * (Fabs + 1e-3 * Fabs.max())).all()
+            for i in range(4):
+                assert rel_linf(st[i].cpu().numpy(), so[i]) <= TOL_STAGE
+        ctx.close()
