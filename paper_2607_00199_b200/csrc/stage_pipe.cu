@@ -56,16 +56,17 @@ struct Cfg {
   // flux tasks at N=4) and the ring has 4 slots (a 5th costs more in L1 capacity than it gains).  2-D: a quad is a
   // few hundred doubles and 36 DMMA per item, the per-quad latency chain of the producers (indices -> copies ->
   // barrier -> flux) is what bounds the kernel (profiles/r1_v12_cfg3_stage_kernel.md), so every producer warp
-  // streams quads of its own (warp w takes quads w, w+6, ...) into a 16-slot ring.
+  // streams quads of its own (warp w takes quads w, w+6, ...) into a 16-slot ring.  3-D N <= 3 sits in between:
+  // two groups of two warps, ring of 8 (config 5: stage kernel 4.94 -> 4.56 ms).
 #ifdef ALEGB_PG
   static constexpr int PG = ALEGB_PG;
 #else
-  static constexpr int PG = DIM == 2 ? 32 : PW * 32;   // threads of one producer group
+  static constexpr int PG = DIM == 2 ? 32 : (N <= 3 ? 64 : PW * 32);   // threads of one producer group
 #endif
 #ifdef ALEGB_NS
   static constexpr int NS = ALEGB_NS;
 #else
-  static constexpr int NS = PG == 32 ? 16 : 4;         // slots in the ring
+  static constexpr int NS = PG == 32 ? 16 : (PG == 64 ? 8 : 4);   // slots in the ring
 #endif
   static constexpr int NG = PW * 32 / PG;      // producer groups
   static constexpr int TAG0 = PG >= 64 ? 32 : EG;   // first thread of a group that fetches boundary tags
