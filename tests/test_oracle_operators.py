@@ -178,3 +178,28 @@ def test_interpolation_matrix_is_barycentric(dim, N, refs):
     f_vert = vref @ coef + 0.11
     assert np.allclose(ref.lam @ f_vert, ref.x @ coef + 0.11, atol=1e-15)
     assert ref.fmask.shape == (dim + 1, {2: N + 1, 3: (N + 1) * (N + 2) // 2}[dim])
+
+
+def test_interior_orbit_of_order_4_matches_survey_values():
+    """SURVEY 8(c)-S1 prints the only nodes of the four (dim, N) pairs of the configs that are not fixed by symmetry
+    and the LGL edge points: the 3-node interior orbit of the 2-D N=4 set, barycentric (0.551583507555,
+    0.224208246222, 0.224208246222) at alpha = 0.1001, and the same orbit on every face of the 3-D N=4 set,
+    (0.551583572091, 0.224208213955, 0.224208213955) at alpha = 0.1002 (reading R10).  A wrong blend
+    exponent, a dropped factor in 4 lambda_a lambda_b or another alpha moves these digits (alpha = 0 gives 0.551551)."""
+    lam = nodes.warp_blend_barycentric(2, 4)
+    lat = nodes.lattice(2, 4)
+    interior = lam[np.all(lat > 0, axis=1)]
+    assert interior.shape == (3, 3)
+    for row in interior:
+        assert np.allclose(np.sort(row), [0.224208246222, 0.224208246222, 0.551583507555], rtol=0, atol=2e-12)
+    lam3 = nodes.warp_blend_barycentric(3, 4)
+    lat3 = nodes.lattice(3, 4)
+    for face in range(4):                                    # the face opposite vertex `face`
+        on_face = lat3[:, face] == 0
+        inner = on_face & (np.sum(lat3 > 0, axis=1) == 3)    # not on an edge of that face
+        assert inner.sum() == 3
+        for row in lam3[inner]:
+            assert np.allclose(np.sort(row), [0.0, 0.224208213955, 0.224208213955, 0.551583572091], rtol=0, atol=2e-12)
+    # sensitivity: the pinned digits separate alpha = 0.1001 from alpha = 0 and from a blend without the square
+    lam0 = nodes.warp_blend_barycentric(2, 4, alpha=0.0)
+    assert abs(np.sort(lam0[np.all(lat > 0, axis=1)][0])[-1] - 0.551583507555) > 1e-5

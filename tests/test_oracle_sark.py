@@ -78,3 +78,68 @@ def test_scalar_fourth_order():
     errs = [abs(scalar_sark(lam, f, q0, 1.0 / n, n) - exact) for n in (8, 16, 32)]
     rates = [np.log2(errs[i] / errs[i + 1]) for i in range(2)]
     assert all(r > 3.7 for r in rates), (errs, rates)
+
+
+# ------------------------------------------------------------------ the stage recurrence of sark.step_debug itself
+class _LinearSystem:
+    """A stand-in for oracle.rhs.Problem with F(q, t) = M q + g(t), M dense: every field feeds every other, so each
+    F_nj differs from the others and from stage to stage (unlike free stream / uniform relaxation, where all F_nj are
+    equal and only the row sums of a~ are exercised)."""
+    dim, sigma = 2, None
+
+    def __init__(self, tau, seed=3):
+        rng = np.random.default_rng(seed)
+        self.tau = tau
+        self.M = rng.uniform(-1, 1, size=(6, 6))
+        self.gv = rng.uniform(-1, 1, size=(6, 3))
+
+    def g(self, t):
+        return self.gv[:, 0] * np.sin(3 * t) + self.gv[:, 1] * np.cos(2 * t) + self.gv[:, 2] * t
+
+    def rhs(self, q, t, verts=None):
+        return np.einsum("fg,kgi->kfi", self.M, q) + self.g(t)[None, :, None]
+
+
+@pytest.mark.parametrize("tau", [0.1, 0.05])
+def test_step_recurrence_is_fourth_order_on_a_coupled_stiff_system(tau):
+    """PAPER.md:L132-134 with the coefficients of L148: q' = -Lambda q + M q + g(t), Lambda = diag(0,0,0,1/tau x3),
+    integrated by oracle.sark.step with |gamma| = dt/tau between 2 and 0.125, against an adaptive high-order
+    integration of the same ODE (scipy DOP853, rtol 1e-13).  The error must fall 16-fold per halving of dt, for the
+    stiff fields on their own too.  a~_20 and a~_21 applied to the wrong F_nj (or a wrong exponent e^{-Lambda c_i dt})
+    leave free stream and uniform relaxation intact but drop this to second order (ratio 4)."""
+    from scipy.integrate import solve_ivp
+    from oracle import physics
+    P = _LinearSystem(tau)
+    lam = physics.stiff_mask(2) / tau
+    q0 = np.linspace(0.5, 1.5, 6)
+    T = 0.8
+    sol = solve_ivp(lambda t, y: -lam * y + P.M @ y + P.g(t), (0, T), q0, method="DOP853", rtol=1e-13, atol=1e-15)
+    exact = sol.y[:, -1]
+    errs = np.array([np.abs(sark.step(P, q0[None, :, None].copy(), 0.0, T / n, n)[0, :, 0] - exact) for n in (8, 16, 32, 64)])
+    for sel in (slice(None), slice(3, 6)):
+        e = errs[:, sel].max(axis=1)
+        assert all(e[i] / e[i + 1] >= 14.0 for i in range(3)), e
+    assert errs[-1].max() < 1e-7                             # error constant of a 4th-order scheme, not just its slope
+
+
+def test_step_temporal_self_convergence_on_a_moving_mesh(refs):
+    """oracle.sark.step on the real operator (2-D, N=2, SINES_PRODUCT motion, finite tau with gamma = -1 at the
+    coarsest dt, second moments away from equilibrium): errors at dt, dt/2, dt/4 against the dt/8 run fall by >= 14
+    per halving (geometry re-evaluated at every stage time, L152-154)."""
+    from helpers import oracle_problem
+    from workloads import configs
+    ref = refs(2, 2)
+    cfg = configs.config2(ref.lam, n=4)
+    cfg["N"] = 2
+    cfg = configs._finish(cfg, ref.lam)
+    dt0 = cfg["dt"]
+    cfg["tau"] = dt0
+    P = oracle_problem(cfg, ref)
+    q0 = cfg["q0"].copy()
+    q0[:, 3:] += 0.02 * np.sin(configs.node_coordinates(cfg["X0"], cfg["EToV"], ref.lam)[..., 0])[:, None, :]
+    T = 8 * dt0
+    outs = [sark.step(P, q0, 0.1, T / n, n) for n in (8, 16, 32, 64)]
+    for sel in (slice(None), slice(3, 6)):
+        e = [np.abs(o - outs[-1])[:, sel].max() for o in outs[:-1]]
+        assert e[0] / e[1] >= 14.0 and e[1] / e[2] >= 14.0, e
+        assert e[2] > 1e-13                                  # still above round-off: the ratios mean something
