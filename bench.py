@@ -188,8 +188,8 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5],
                     help="BASELINE.json workload (1-based); 4 = the 3D N=4 throughput configuration")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--kernel", type=int, default=0, choices=[0, 1, 2, 3],
-                    help="alegb_set_kernel: 0 auto, 1 generic DFMA, 2 pipelined DMMA, 3 warp-per-quad DMMA")
+    ap.add_argument("--kernel", type=int, default=0, choices=[0, 1, 2],
+                    help="alegb_set_kernel: 0 auto, 1 generic DFMA, 2 pipelined DMMA")
     ap.add_argument("--relax", default="collocation", choices=["collocation", "cubature"],
                     help="nonlinear relaxation: collocated (default, DESIGN.md R8) or cubature-projected (NEXT-1)")
     ap.add_argument("--coords", default="closed", choices=["closed", "rk"],

@@ -188,10 +188,19 @@ const char* alegb_last_error(const alegb_ctx* ctx);
 /* number of kernel launches the library has enqueued on this context since creation */
 int64_t alegb_launch_count(const alegb_ctx* ctx);
 /* Which fused stage kernel runs: 0 = automatic (the pipelined tensor-core DMMA kernel where one is compiled for
- * (dim, N), the generic kernel otherwise), 1 = generic element-blocked DFMA kernel, 2 = pipelined DMMA kernel
- * (producer/consumer warps), 3 = warp-per-4-elements DMMA kernel; 2 and 3 return ALEGB_UNSUPPORTED if there is none.
- * All compute the same operator; tests run all of them. */
+ * (dim, N), the generic kernel otherwise), 1 = generic element-blocked DFMA kernel (every (dim, N); kept as an
+ * independent implementation of the same operator), 2 = pipelined DMMA kernel (producer/consumer warps; returns
+ * ALEGB_UNSUPPORTED if there is none for (dim, N)).  Tests run both. */
 int alegb_set_kernel(alegb_ctx* ctx, int kind);
+/* Cap on the number of CTAs of the persistent kernels (stage, absorbing layer, cubature): 0 = one per SM (default).
+ * A tuning / test knob: with few CTAs every CTA walks through many work units, which is the regime in which the
+ * shared-memory ring of the pipelined kernel wraps many times.  Results do not depend on it. */
+int alegb_set_max_ctas(alegb_ctx* ctx, int max_ctas);
+/* Hand-over parameters of the pipelined stage kernel compiled for (dim, N), HOST out cfg[8] = {producer groups,
+ * ring slots, work items per quad, consumer warps, warps per producer group, producer warps, elements per quad,
+ * dynamic shared memory in bytes}.  ALEGB_UNSUPPORTED if there is no such kernel.  Needs no context and no device
+ * (tests/test_pipe_protocol.py simulates the protocol with these numbers). */
+int alegb_pipe_config(int dim, int N, int* cfg);
 /* Inside a step the vertex-motion and geometric-factor kernels (a1, a2) of stage i+1 depend on time only; with the
  * overlap on (default) they run on a stream of the library's own beside the stage kernel of stage i, into a second
  * set of geometry arrays, joined by events (captured into the step graph as a parallel branch).  Same kernels, same
@@ -209,7 +218,9 @@ int alegb_set_graph(alegb_ctx* ctx, int on);
 int alegb_profile_enable(alegb_ctx* ctx, int on);
 int alegb_profile_read(alegb_ctx* ctx, int64_t* launches, double* total_ms);
 /* Synchronous convenience entry for host buffers (HOST q [K][Nf][Np], updated in place): copies q to the device,
- * runs nsteps SARK4 steps, copies the result back, synchronises.  Used for end-to-end timing. */
+ * runs nsteps SARK4 steps, copies the result back.  Everything is enqueued on the LEGACY DEFAULT STREAM (stream 0),
+ * which the call synchronises before it returns; the whole state crosses PCIe twice per call, so the cost per step
+ * falls with nsteps (one step per call is bound by the two copies, not by the kernels).  Used for end-to-end timing. */
 int alegb_step_host(alegb_ctx* ctx, double* h_q, double t0, double dt, int nsteps);
 
 #define ALEGB_MAX_N 5

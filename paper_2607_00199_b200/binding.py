@@ -57,6 +57,8 @@ _SIGNATURES = {
     "alegb_last_error": (_c.c_char_p, [_P]),
     "alegb_launch_count": (_c.c_int64, [_P]),
     "alegb_set_kernel": (_c.c_int, [_P, _c.c_int]),
+    "alegb_set_max_ctas": (_c.c_int, [_P, _c.c_int]),
+    "alegb_pipe_config": (_c.c_int, [_c.c_int, _c.c_int, _P]),
     "alegb_set_graph": (_c.c_int, [_P, _c.c_int]),
     "alegb_profile_enable": (_c.c_int, [_P, _c.c_int]),
     "alegb_profile_read": (_c.c_int, [_P, _c.POINTER(_c.c_int64), _c.POINTER(_c.c_double)]),
@@ -81,6 +83,8 @@ def _dev(x):
         return x
     if not x.is_cuda or not x.is_contiguous():
         raise ValueError("device arrays must be contiguous CUDA tensors")
+    if str(x.dtype) != "torch.float64":
+        raise ValueError("device arrays must be float64 (got %s)" % x.dtype)
     return x.data_ptr()
 
 
@@ -256,6 +260,9 @@ class Context:
     def alegb_set_kernel(self, kind):
         self._check(_lib.alegb_set_kernel(self._h, int(kind)))
 
+    def alegb_set_max_ctas(self, max_ctas):
+        self._check(_lib.alegb_set_max_ctas(self._h, int(max_ctas)))
+
     def alegb_set_graph(self, on):
         self._check(_lib.alegb_set_graph(self._h, int(bool(on))))
 
@@ -278,6 +285,19 @@ def alegb_sark_coefficients(gamma):
     if rc != OK:
         raise AlegbError(rc, "alegb_sark_coefficients")
     return a, b
+
+
+PIPE_CONFIG_FIELDS = ("producer_groups", "slots", "items_per_quad", "consumer_warps", "warps_per_group",
+                      "producer_warps", "elements_per_quad", "smem_bytes")
+
+
+def alegb_pipe_config(dim, N):
+    """-> dict of the hand-over parameters of the pipelined stage kernel for (dim, N); raises UNSUPPORTED if none."""
+    out = (_c.c_int * 8)()
+    rc = _lib.alegb_pipe_config(int(dim), int(N), out)
+    if rc != OK:
+        raise AlegbError(rc, "alegb_pipe_config(dim=%d, N=%d)" % (dim, N))
+    return dict(zip(PIPE_CONFIG_FIELDS, (int(v) for v in out)))
 
 
 def context_from_config(cfg, cuda_device=0):

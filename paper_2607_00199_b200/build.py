@@ -21,7 +21,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 CXX_FLAGS = ["-O2", "-std=c++17", "-fPIC"]
 
-CU_SOURCES = ["kernels.cu", "stage_mma.cu", "stage_pipe.cu", "pml_mma.cu", "cubature.cu", "alegb_api.cu"]
+CU_SOURCES = ["kernels.cu", "stage_pipe.cu", "pml_mma.cu", "cubature.cu", "alegb_api.cu"]
 CXX_SOURCES = ["host_ref.cpp"]
 HEADERS = ["alegb_internal.h", "device_common.cuh", "host_ref.h", os.path.join("..", "..", "include", "alegb.h")]
 
@@ -61,10 +61,6 @@ def build(force=False, verbose=False):
         objs.append(o)
     if force or _newer(LIB, objs):
         _run([NVCC, "-shared", "-o", LIB] + objs + ["-lquadmath"], verbose, log)
-    for tool in ("fp64_peak", "fp64_arbitration"):   # stand-alone microbenchmarks (profiles/r1_fp64_*.md)
-        src, exe = os.path.join(CSRC, tool + ".cu"), os.path.join(HERE, tool)
-        if os.path.exists(src) and (force or _newer(exe, [src])):
-            _run([NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", exe, src], verbose, log)
     with open(os.path.join(OBJ, "build.log"), "a") as f:
         f.write("\n".join(log))
     return LIB

@@ -1,5 +1,6 @@
 // C-ABI entry points (include/alegb.h): context management, mesh upload, the stage loop of the SARK4 step.
-// Host logic only: every arithmetic step of the path runs in the kernels of kernels.cu / stage_mma.cu.
+// Host logic only: every arithmetic step of the path runs in the kernels of kernels.cu / stage_pipe.cu / pml_mma.cu /
+// cubature.cu.
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -12,7 +13,8 @@
 using namespace alegb;
 
 struct alegb_ctx {
-  int device = 0, num_sms = 0;
+  int device = 0, num_sms = 0, max_ctas = 0;   // max_ctas: alegb_set_max_ctas (0 = one CTA per SM)
+  int ctas() const { return max_ctas > 0 && max_ctas < num_sms ? max_ctas : num_sms; }
   RefElement ref;
   int Nf = 0;
   int64_t K = 0, Nverts = 0, Kpml = 0;
@@ -22,13 +24,13 @@ struct alegb_ctx {
   MotionArgs motion{};
   std::vector<int32_t> vmapM_host, vmapP_host, pml_elems_host;
   // device: operators
-  double *d_Dt = nullptr, *d_LIFTt = nullptr, *d_lam = nullptr, *d_Avol = nullptr, *d_Alift = nullptr, *d_AliftP = nullptr;
+  double *d_Dt = nullptr, *d_LIFTt = nullptr, *d_lam = nullptr, *d_Avol = nullptr, *d_AliftP = nullptr;
   int32_t* d_fmask = nullptr;
   double *d_wface = nullptr, *d_force = nullptr;   // NEXT-3: face quadrature weights; partial sums + result
-  bool mma_ok = false;   // a warp-per-quad DMMA stage kernel exists for (dim, N)
+  bool cub_mma_ok = false;  // a DMMA cubature kernel exists for (dim, N)
   bool pipe_ok = false;  // a pipelined DMMA stage kernel exists for (dim, N)
   bool pml_mma_ok = false;  // a DMMA kernel for the absorbing layer's auxiliary fields exists for (dim, N)
-  int kernel_mode = 0;   // 0 auto (pipelined DMMA, else DMMA, else generic), 1 generic, 2 pipelined DMMA, 3 warp-per-quad DMMA
+  int kernel_mode = 0;   // 0 auto (pipelined DMMA, else generic), 1 generic, 2 pipelined DMMA
   // device: mesh
   double *d_X0 = nullptr, *d_xv = nullptr, *d_vv = nullptr;
   // NEXT-2: coordinates integrated by RK4: current positions x_n, the user's constant velocity
@@ -159,7 +161,7 @@ void fill_common(const alegb_ctx* ctx, StageArgs& a) {
   a.vmapP = ctx->d_vmapP; a.EToB = ctx->d_EToB;
   a.pml_index = ctx->d_pml_index; a.pml_sigma = ctx->d_pml_sigma;
   a.Dt_ops = ctx->d_Dt; a.LIFTt = ctx->d_LIFTt; a.lam = ctx->d_lam; a.fmask = ctx->d_fmask;
-  a.Avol = ctx->d_Avol; a.Alift = ctx->d_Alift; a.AliftP = ctx->d_AliftP;
+  a.Avol = ctx->d_Avol; a.AliftP = ctx->d_AliftP;
   a.c = ctx->c; a.invtau = ctx->invtau;
   for (int k = 0; k < kMaxFields; ++k) a.q_inf[k] = ctx->q_inf[k];
 }
@@ -175,8 +177,8 @@ void fill_common(const alegb_ctx* ctx, PmlArgs& a) {
 }
 // a8: the DMMA kernel unless the generic kernels were asked for (alegb_set_kernel(1)) or (dim, N) has none
 cudaError_t launch_pml_any(const alegb_ctx* ctx, const PmlArgs& p, cudaStream_t s) {
-  if (ctx->pml_mma_ok && ctx->kernel_mode != 1) return launch_pml_mma(ctx->ref.dim, ctx->ref.N, p, ctx->num_sms, s);
-  return launch_pml(ctx->ref.dim, ctx->ref.N, p, ctx->num_sms, s);
+  if (ctx->pml_mma_ok && ctx->kernel_mode != 1) return launch_pml_mma(ctx->ref.dim, ctx->ref.N, p, ctx->ctas(), s);
+  return launch_pml(ctx->ref.dim, ctx->ref.N, p, ctx->ctas(), s);
 }
 
 int check_ready(alegb_ctx* ctx) {
@@ -192,18 +194,7 @@ int check_ready(alegb_ctx* ctx) {
 // the fused stage kernel, bracketed by events while profiling is enabled
 int timed_stage(alegb_ctx* ctx, const StageArgs& a_in, cudaStream_t s) {
   StageArgs a = a_in;
-  if (ctx->relax_mode == ALEGB_RELAX_CUBATURE) {
-    // kernel v of the paper (L197): R = P N~(I q_in), read by the stage kernel in place of the collocated N~
-    CubArgs cb;
-    cb.K = ctx->K; cb.Np = ctx->ref.Np; cb.Nc = ctx->cub.Nc; cb.EB = ctx->cub_EB;
-    cb.It = ctx->d_It; cb.Pt = ctx->d_Pt; cb.AI = ctx->d_AI; cb.AP = ctx->d_AP;
-    cb.q = a.q_in; cb.R = ctx->d_R; cb.invtau = ctx->invtau;
-    // kernel kind 1 (generic DFMA stage kernel) keeps the DFMA cubature kernel: two independent implementations
-    if (ctx->kernel_mode == 1) CU(launch_cubature(ctx->ref.dim, cb, ctx->num_sms, s));
-    else CU(launch_cubature_mma(ctx->ref.dim, ctx->ref.N, cb, ctx->num_sms, s));
-    ctx->launches++;
-    a.relax_cub = ctx->d_R;
-  }
+  // profiling brackets everything the stage launches (the cubature kernel of the optional mode included)
   const bool rec = ctx->profiling && ctx->prof_used + 2 <= 8192;
   if (rec) {
     while (ctx->prof_events.size() < ctx->prof_used + 2) {
@@ -213,10 +204,22 @@ int timed_stage(alegb_ctx* ctx, const StageArgs& a_in, cudaStream_t s) {
     }
     CU(cudaEventRecord(ctx->prof_events[ctx->prof_used], s));
   }
+  if (ctx->relax_mode == ALEGB_RELAX_CUBATURE) {
+    // kernel v of the paper (L197): R = P N~(I q_in), read by the stage kernel in place of the collocated N~
+    CubArgs cb;
+    cb.K = ctx->K; cb.Np = ctx->ref.Np; cb.Nc = ctx->cub.Nc; cb.EB = ctx->cub_EB;
+    cb.It = ctx->d_It; cb.Pt = ctx->d_Pt; cb.AI = ctx->d_AI; cb.AP = ctx->d_AP;
+    cb.q = a.q_in; cb.R = ctx->d_R; cb.invtau = ctx->invtau;
+    // kernel kind 1 (generic DFMA stage kernel) keeps the DFMA cubature kernel: two independent implementations;
+    // it is also the only one for a (dim, N) without a DMMA cubature kernel (3-D N = 5)
+    if (ctx->kernel_mode == 1 || !ctx->cub_mma_ok) CU(launch_cubature(ctx->ref.dim, cb, ctx->ctas(), s));
+    else CU(launch_cubature_mma(ctx->ref.dim, ctx->ref.N, cb, ctx->ctas(), s));
+    ctx->launches++;
+    a.relax_cub = ctx->d_R;
+  }
   const int mode = ctx->kernel_mode;
-  if (ctx->pipe_ok && (mode == 0 || mode == 2)) CU(launch_stage_pipe(ctx->ref.dim, ctx->ref.N, a, ctx->num_sms, s));
-  else if (ctx->mma_ok && (mode == 0 || mode == 3)) CU(launch_stage_mma(ctx->ref.dim, ctx->ref.N, a, ctx->num_sms, s));
-  else CU(launch_stage(ctx->ref.dim, ctx->ref.N, a, ctx->num_sms, s));
+  if (ctx->pipe_ok && (mode == 0 || mode == 2)) CU(launch_stage_pipe(ctx->ref.dim, ctx->ref.N, a, ctx->ctas(), s));
+  else CU(launch_stage(ctx->ref.dim, ctx->ref.N, a, ctx->ctas(), s));
   ctx->launches++;
   if (rec) {
     CU(cudaEventRecord(ctx->prof_events[ctx->prof_used + 1], s));
@@ -421,13 +424,12 @@ int alegb_create(alegb_ctx** out, int dim, int N, int cuda_device) {
     for (int m = 0; m < ncol; ++m) Lt[(size_t)m * Np + i] = r.LIFT[i * ncol + m];
   std::vector<int32_t> fm(r.fmask.begin(), r.fmask.end());
   // operators in DMMA fragment order: lane l of fragment (row tile nb, k-step ks) holds A[8 nb + l/4][4 ks + l%4]
-  MmaLayout L{};
-  ctx->mma_ok = mma_layout(dim, N, L) && configure_stage_mma(dim, N) == cudaSuccess;
-  ctx->pipe_ok = ctx->mma_ok && configure_stage_pipe(dim, N) == cudaSuccess;
-  ctx->pml_mma_ok = ctx->mma_ok && configure_pml_mma(dim, N) == cudaSuccess;
+  struct { int NB, KS; } L{(Np + 7) / 8, (Np + 3) / 4};   // node blocks of 8 rows, k-steps of 4 columns
+  ctx->pipe_ok = configure_stage_pipe(dim, N) == cudaSuccess;
+  ctx->pml_mma_ok = configure_pml_mma(dim, N) == cudaSuccess;
   cudaGetLastError();
-  if (ctx->mma_ok) {
-    std::vector<double> Av((size_t)dim * L.NB * L.KS * 32, 0.0), Al((size_t)r.Nfaces * L.NB * L.KF * 32, 0.0);
+  if (ctx->pipe_ok || ctx->pml_mma_ok) {
+    std::vector<double> Av((size_t)dim * L.NB * L.KS * 32, 0.0);
     for (int a = 0; a < dim; ++a)
       for (int nb = 0; nb < L.NB; ++nb)
         for (int ks = 0; ks < L.KS; ++ks)
@@ -435,14 +437,7 @@ int alegb_create(alegb_ctx** out, int dim, int N, int cuda_device) {
             const int row = 8 * nb + l / 4, col = 4 * ks + l % 4;
             if (row < Np && col < Np) Av[(((size_t)a * L.NB + nb) * L.KS + ks) * 32 + l] = r.D[a][row * Np + col];
           }
-    for (int f = 0; f < r.Nfaces; ++f)
-      for (int nb = 0; nb < L.NB; ++nb)
-        for (int ks = 0; ks < L.KF; ++ks)
-          for (int l = 0; l < 32; ++l) {
-            const int row = 8 * nb + l / 4, m = 4 * ks + l % 4;
-            if (row < Np && m < r.Nfp) Al[(((size_t)f * L.NB + nb) * L.KF + ks) * 32 + l] = r.LIFT[row * ncol + f * r.Nfp + m];
-          }
-    const int KFT = (ncol + 3) / 4;   // pipelined kernel: the faces' k ranges packed back to back, m = f*Nfp + mm
+    const int KFT = (ncol + 3) / 4;   // the faces' k ranges packed back to back, m = f*Nfp + mm
     std::vector<double> Alp((size_t)L.NB * KFT * 32, 0.0);
     for (int nb = 0; nb < L.NB; ++nb)
       for (int ks = 0; ks < KFT; ++ks)
@@ -451,7 +446,6 @@ int alegb_create(alegb_ctx** out, int dim, int N, int cuda_device) {
           if (row < Np && m < ncol) Alp[((size_t)nb * KFT + ks) * 32 + l] = r.LIFT[row * ncol + m];
         }
     if (upload(ctx, &ctx->d_Avol, Av.data(), Av.size()) != cudaSuccess ||
-        upload(ctx, &ctx->d_Alift, Al.data(), Al.size()) != cudaSuccess ||
         upload(ctx, &ctx->d_AliftP, Alp.data(), Alp.size()) != cudaSuccess) {
       alegb_destroy(ctx);
       return ALEGB_CUDA_ERROR;
@@ -488,7 +482,8 @@ int alegb_destroy(alegb_ctx* ctx) {
   for (cudaEvent_t ev : ctx->prof_events) cudaEventDestroy(ev);
   dev_free(ctx->d_Dt); dev_free(ctx->d_LIFTt); dev_free(ctx->d_lam); dev_free(ctx->d_fmask);
   dev_free(ctx->d_wface); dev_free(ctx->d_force);
-  dev_free(ctx->d_Avol); dev_free(ctx->d_Alift); dev_free(ctx->d_AliftP);
+  dev_free(ctx->d_Avol); dev_free(ctx->d_AliftP);
+  dev_free(ctx->d_It); dev_free(ctx->d_Pt); dev_free(ctx->d_AI); dev_free(ctx->d_AP);
   delete ctx;
   return ALEGB_OK;
 }
@@ -662,7 +657,8 @@ int alegb_set_relaxation(alegb_ctx* ctx, int mode) {
       CU(dev_alloc(ctx, &ctx->d_Pt, Pt.size()));
       CU(cudaMemcpy(ctx->d_It, It.data(), It.size() * sizeof(double), cudaMemcpyHostToDevice));
       CU(cudaMemcpy(ctx->d_Pt, Pt.data(), Pt.size() * sizeof(double), cudaMemcpyHostToDevice));
-      {   // A-fragment order: lane l of fragment (row tile, k-step) holds A[8 tile + l/4][4 k + l%4], zero outside
+      ctx->cub_mma_ok = cubature_mma_available(dim, ctx->ref.N);
+      if (ctx->cub_mma_ok) {   // A-fragment order: lane l of fragment (row tile, k-step) holds A[8 tile + l/4][4 k + l%4], zero outside
         int NRT, KS, NB;
         cubature_mma_layout(dim, ctx->ref.N, NRT, KS, NB);
         std::vector<double> AI((size_t)NRT * KS * 32, 0.0), AP((size_t)NB * 2 * NRT * 32, 0.0);
@@ -938,11 +934,27 @@ int alegb_sark_coefficients(double gamma, double* a, double* b) {
 
 int alegb_set_kernel(alegb_ctx* ctx, int kind) {
   if (!ctx) return ALEGB_INVALID_ARG;
-  if (kind < 0 || kind > 3) return fail(ctx, ALEGB_INVALID_ARG, "kernel kind must be 0 (auto), 1 (generic), 2 (pipelined DMMA) or 3 (warp-per-quad DMMA)");
+  if (kind < 0 || kind > 2) return fail(ctx, ALEGB_INVALID_ARG, "kernel kind must be 0 (auto), 1 (generic) or 2 (pipelined DMMA)");
   if (kind == 2 && !ctx->pipe_ok) return fail(ctx, ALEGB_UNSUPPORTED, "no pipelined DMMA stage kernel for this (dim, N)");
-  if (kind == 3 && !ctx->mma_ok) return fail(ctx, ALEGB_UNSUPPORTED, "no DMMA stage kernel for this (dim, N)");
   ctx->kernel_mode = kind;
   ctx->config_version++;
+  return ALEGB_OK;
+}
+
+int alegb_set_max_ctas(alegb_ctx* ctx, int max_ctas) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  if (max_ctas < 0) return fail(ctx, ALEGB_INVALID_ARG, "max_ctas must be >= 0 (0 = one CTA per SM)");
+  ctx->max_ctas = max_ctas;
+  ctx->config_version++;
+  return ALEGB_OK;
+}
+
+int alegb_pipe_config(int dim, int N, int* cfg) {
+  if (!cfg) return ALEGB_INVALID_ARG;
+  PipeConfig c{};
+  if (!stage_pipe_config(dim, N, c)) return ALEGB_UNSUPPORTED;
+  cfg[0] = c.producer_groups; cfg[1] = c.slots; cfg[2] = c.items_per_quad; cfg[3] = c.consumer_warps;
+  cfg[4] = c.warps_per_group; cfg[5] = c.producer_warps; cfg[6] = c.elements_per_quad; cfg[7] = c.smem_bytes;
   return ALEGB_OK;
 }
 

@@ -42,8 +42,7 @@ struct StageArgs {
   const double* lam;     // [Np][dim+1]
   const int32_t* fmask;  // [Nfaces*Nfp]
   const double* Avol;    // DMMA path: D_a in fragment order [dim][NB][KS][32]
-  const double* Alift;   // DMMA path: LIFT in fragment order [Nfaces][NB][KF][32]
-  const double* AliftP;  // DMMA path, faces packed along k: [NB][ceil(Nfaces*Nfp/4)][32]
+  const double* AliftP;  // DMMA path: LIFT in fragment order, faces packed along k: [NB][ceil(Nfaces*Nfp/4)][32]
   // physics
   double c, invtau;
   const double* relax_cub;   // R = P N~(I q) [K][Ns][Np] replacing the collocated N~(q), or NULL (reading R8)
@@ -123,13 +122,8 @@ size_t cubature_smem_bytes(int dim, int Np, int Nc, int EB);
 cudaError_t configure_cubature(int dim, size_t smem);
 cudaError_t launch_cubature(int dim, const CubArgs& a, int num_sms, cudaStream_t s);
 void cubature_mma_layout(int dim, int N, int& NRT, int& KS, int& NB);   // fragment-array extents
+bool cubature_mma_available(int dim, int N);
 cudaError_t launch_cubature_mma(int dim, int N, const CubArgs& a, int num_sms, cudaStream_t s);   // InvalidValue: none for (dim, N)
-
-// tensor-core (DMMA) stage kernel, stage_mma.cu
-struct MmaLayout { int NB, KS, KF; };               // node blocks, k-steps of the volume / per-face contraction
-bool mma_layout(int dim, int N, MmaLayout& L);       // false if (dim, N) has no DMMA kernel
-cudaError_t configure_stage_mma(int dim, int N);
-cudaError_t launch_stage_mma(int dim, int N, const StageArgs& a, int num_sms, cudaStream_t s);
 
 // tensor-core kernel of the absorbing layer's auxiliary fields, pml_mma.cu
 cudaError_t configure_pml_mma(int dim, int N);        // cudaErrorInvalidValue if (dim, N) has no such kernel
@@ -138,5 +132,7 @@ cudaError_t launch_pml_mma(int dim, int N, const PmlArgs& a, int num_sms, cudaSt
 // pipelined tensor-core stage kernel (producer / consumer warps), stage_pipe.cu; same operator fragments
 cudaError_t configure_stage_pipe(int dim, int N);     // cudaErrorInvalidValue if (dim, N) has no such kernel
 cudaError_t launch_stage_pipe(int dim, int N, const StageArgs& a, int num_sms, cudaStream_t s);
+struct PipeConfig { int producer_groups, slots, items_per_quad, consumer_warps, warps_per_group, producer_warps, elements_per_quad, smem_bytes; };
+bool stage_pipe_config(int dim, int N, PipeConfig& c);   // false if (dim, N) has no such kernel
 
 }  // namespace alegb

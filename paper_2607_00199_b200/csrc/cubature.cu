@@ -244,6 +244,10 @@ void cubature_mma_layout(int dim, int N, int& NRT, int& KS, int& NB) {
   NRT = (Nc + 7) / 8; KS = (Np + 3) / 4; NB = (Np + 7) / 8;
 }
 
+bool cubature_mma_available(int dim, int N) {   // the (dim, N) pairs launch_cubature_mma dispatches
+  return (dim == 2 && N >= 1 && N <= 5) || (dim == 3 && N >= 1 && N <= 4);
+}
+
 cudaError_t launch_cubature_mma(int dim, int N, const CubArgs& a, int num_sms, cudaStream_t s) {
   switch (dim * 10 + N) {
     case 21: return launch_cub_mma_one<2, 1>(a, num_sms, s);

@@ -5,7 +5,7 @@
 //   a3-a6 stage_kernel         volume + collocated relaxation + surface + SARK stage update, fused (L107, L132-134)
 //   a8  pml_kernel             auxiliary fields of the absorbing layer (reading R12)
 //
-// The tensor-core (DMMA) specialisations of the stage kernel live in stage_mma.cu.
+// The tensor-core (DMMA) stage kernel lives in stage_pipe.cu.
 #include <cstdio>
 
 #include "alegb_internal.h"

@@ -19,10 +19,6 @@
 #include "alegb_internal.h"
 #include "device_common.cuh"
 
-#ifndef ALEGB_DBG
-#define ALEGB_DBG 0   // timing experiments only: bit mask of phases to skip (results are then wrong)
-#endif
-
 namespace alegb {
 
 namespace pipe {
@@ -58,16 +54,8 @@ struct Cfg {
   // barrier -> flux) is what bounds the kernel (profiles/r1_v12_cfg3_stage_kernel.md), so every producer warp
   // streams quads of its own (warp w takes quads w, w+6, ...) into a 16-slot ring.  3-D N <= 3 sits in between:
   // two groups of two warps, ring of 8 (config 5: stage kernel 4.94 -> 4.56 ms).
-#ifdef ALEGB_PG
-  static constexpr int PG = ALEGB_PG;
-#else
   static constexpr int PG = DIM == 2 ? 32 : (N <= 3 ? 64 : PW * 32);   // threads of one producer group
-#endif
-#ifdef ALEGB_NS
-  static constexpr int NS = ALEGB_NS;
-#else
   static constexpr int NS = PG == 32 ? 16 : (PG == 64 ? 8 : 4);   // slots in the ring
-#endif
   static constexpr int NG = PW * 32 / PG;      // producer groups
   static constexpr int TAG0 = PG >= 64 ? 32 : EG;   // first thread of a group that fetches boundary tags
   static constexpr int Threads = (PW + CW) * 32;
@@ -270,7 +258,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       producer_sync<PT>(grp);
       // ---- a5: upwind flux at my face nodes (eq. 7; reading R7), in place over the gathered q+
 #pragma unroll
-      for (int r = 0; r < ((ALEGB_DBG & 1) ? 0 : ROUNDS); ++r) {
+      for (int r = 0; r < ROUNDS; ++r) {
         const int fe = task_fe[r], m = task_m[r];
         if (r * PT + pt >= C::NTASK || fe >= nel) continue;
         const int f = m / Nfp;
@@ -352,7 +340,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
 #pragma unroll
         for (int t = 0; t < NT; ++t) acc[d][t][0] = acc[d][t][1] = 0.0;
 #pragma unroll
-      for (int ks = 0; ks < ((ALEGB_DBG & 2) ? 0 : KS); ++ks) {
+      for (int ks = 0; ks < KS; ++ks) {
         double bf[NT], af[DIM];
 #pragma unroll
         for (int t = 0; t < NT; ++t) bf[t] = qt[(bcol + 2 * t) * S + 4 * ks + c];
@@ -367,10 +355,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       const int n = 8 * nb + g;
       const int nn = n < Np ? n : Np - 1;
       double V[NT][2];
-      if constexpr (ALEGB_DBG & 4) {
-#pragma unroll
-        for (int k = 0; k < Nf; ++k) V[k >> 1][k & 1] = acc[0][k >> 1][k & 1] + acc[1][k >> 1][k & 1] + acc[DIM - 1][k >> 1][k & 1];
-      } else {
+      {
         double G[DIM * DIM], w[DIM], vG[DIM];
 #pragma unroll
         for (int x = 0; x < DIM * DIM; ++x) G[x] = svg[x];
@@ -420,7 +405,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       double uq[Nf], uf[Nf], ua[Nf];
 #pragma unroll
       for (int k = 0; k < Nf; ++k) { uq[k] = 0.0; uf[k] = 0.0; ua[k] = 0.0; }
-      if (evalid && want_update && !(ALEGB_DBG & 16)) {
+      if (evalid && want_update) {
         if (qn_in_tile) {
 #pragma unroll
           for (int k = 0; k < Nf; ++k) uq[k] = qt[(c * Nf + k) * S + nn];
@@ -442,7 +427,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       }
       // ---- a5: LIFT contraction of the quad's flux tile into the same registers (L103, L196)
 #pragma unroll
-      for (int ks = 0; ks < ((ALEGB_DBG & 8) ? 0 : KFT); ++ks) {
+      for (int ks = 0; ks < KFT; ++ks) {
         double bf[NT];
 #pragma unroll
         for (int t = 0; t < NT; ++t) bf[t] = gt[(bcol + 2 * t) * SG + 4 * ks + c];
@@ -453,7 +438,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       // all reads of the slot are done
       mbar_arrive(&empty[slot]);
       // ---- a6: SARK stage update (L132-134), straight from the accumulator registers; one uniform branch per output
-      if (evalid && (!(ALEGB_DBG & 32) || V[0][0] == 1.2345e300)) {
+      if (evalid) {
         if (a.F_out != nullptr) {
           double* of = a.F_out + base;
 #pragma unroll
@@ -526,6 +511,31 @@ cudaError_t launch_stage_pipe(int dim, int N, const StageArgs& a, int num_sms, c
 cudaError_t configure_stage_pipe(int dim, int N) {
   StageArgs a{};
   ALEGB_PIPE_DISPATCH(a, 0, nullptr, true)
+}
+
+// The hand-over parameters of Cfg<DIM,N>, for tests/test_pipe_protocol.py (alegb_pipe_config): the simulation must
+// model the kernel that is compiled, not a re-typed copy of its constants.
+template <int DIM, int N>
+static bool pipe_config_one(PipeConfig& c) {
+  using C = pipe::Cfg<DIM, N>;
+  if (!C::supported) return false;
+  c.producer_groups = C::NG; c.slots = C::NS; c.items_per_quad = C::NB; c.consumer_warps = C::CW;
+  c.warps_per_group = C::PG / 32; c.producer_warps = C::PW; c.elements_per_quad = C::EG; c.smem_bytes = (int)C::smem_bytes;
+  return true;
+}
+bool stage_pipe_config(int dim, int N, PipeConfig& c) {
+  switch (dim * 10 + N) {
+    case 21: return pipe_config_one<2, 1>(c);
+    case 22: return pipe_config_one<2, 2>(c);
+    case 23: return pipe_config_one<2, 3>(c);
+    case 24: return pipe_config_one<2, 4>(c);
+    case 25: return pipe_config_one<2, 5>(c);
+    case 31: return pipe_config_one<3, 1>(c);
+    case 32: return pipe_config_one<3, 2>(c);
+    case 33: return pipe_config_one<3, 3>(c);
+    case 34: return pipe_config_one<3, 4>(c);
+    default: return false;
+  }
 }
 
 }  // namespace alegb

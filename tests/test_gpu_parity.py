@@ -66,7 +66,7 @@ def make_case(name, refs):
 
 
 CASES = ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "tri_N1", "tri_N5", "tet_N2", "tet_N5"]
-KERNELS = [1, 2, 3]     # alegb_set_kernel: 1 = generic DFMA kernel, 2 = pipelined DMMA kernel, 3 = warp-per-quad DMMA kernel
+KERNELS = [1, 2]     # alegb_set_kernel: 1 = generic DFMA kernel, 2 = pipelined DMMA kernel
 
 
 def make_ctx(B, cfg, kernel):
@@ -74,7 +74,7 @@ def make_ctx(B, cfg, kernel):
     try:
         ctx.alegb_set_kernel(kernel)
     except B.AlegbError as e:
-        assert e.status == B.UNSUPPORTED and kernel in (2, 3)
+        assert e.status == B.UNSUPPORTED and kernel == 2
         ctx.close()
         pytest.skip("no DMMA kernel for dim=%d N=%d (the generic kernel covers it)" % (cfg["dim"], cfg["N"]))
     return ctx
@@ -433,7 +433,7 @@ def test_rk_coordinates_stage_states_match_oracle(name, refs, B):
         qo, xo = coords.step(P, q, P.X0.copy(), t0, dt, 2)
         auxo = None
     assert np.abs(dx.cpu().numpy() - xo).max() <= 1e-14 * max(1.0, np.abs(xo).max())
-    assert rel_linf(dq.cpu().numpy(), qo) <= 2 * TOL_STAGE
+    assert rel_linf(dq.cpu().numpy(), qo) <= TOL_STAGE
     # the third step observed stage by stage; step_debug must leave x_n alone
     st = torch.empty((4,) + q.shape, dtype=torch.float64, device="cuda")
     ctx.alegb_step_debug(dq, t0 + 2 * dt, dt, st)
@@ -443,7 +443,7 @@ def test_rk_coordinates_stage_states_match_oracle(name, refs, B):
     assert torch.equal(dx, dx2)
     so, _, _ = coords.step_debug(P, qo, xo, t0 + 2 * dt, dt, auxo)
     for i in range(4):
-        assert rel_linf(st[i].cpu().numpy(), so[i]) <= 2 * TOL_STAGE
+        assert rel_linf(st[i].cpu().numpy(), so[i]) <= TOL_STAGE
     ctx.close()
 
 
@@ -500,7 +500,7 @@ def _cubature_case(name, refs):
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("kernel", KERNELS)
-@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "tri_N5", "tet_N2"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "tri_N5", "tet_N2", "tet_N5"])
 def test_cubature_rhs_matches_oracle(name, kernel, refs, B):
     ref, cfg, P = _cubature_case(name, refs)
     ctx = make_ctx(B, cfg, kernel)
@@ -519,6 +519,27 @@ def test_cubature_rhs_matches_oracle(name, kernel, refs, B):
     ctx.alegb_rhs(t, dq, dF2)
     torch.cuda.synchronize()
     assert (dF2 - dF).abs().max().item() > 1e3 * TOL_F * Fabs.max()
+    ctx.close()
+
+
+@pytest.mark.gpu
+def test_cubature_with_automatic_kernel_where_no_dmma_cubature_kernel_exists(refs, B):
+    """3-D N=5 has neither a pipelined stage kernel nor a DMMA cubature kernel: the automatic selection
+    (alegb_set_kernel(0), the default) must fall back to the generic kernels instead of failing."""
+    ref, cfg, P = _cubature_case("tet_N5", refs)
+    ctx = B.context_from_config(cfg)
+    ctx.alegb_set_relaxation(B.RELAX_CUBATURE)
+    q = perturbed(cfg, amp=3e-2)
+    dq, dF = dev(q), torch.empty(q.shape, dtype=torch.float64, device="cuda")
+    ctx.alegb_rhs(0.31, dq, dF)
+    torch.cuda.synchronize()
+    out = P.rhs(q, 0.31, want_abs=True)
+    F, Fabs = out[0], out[-1]
+    assert (np.abs(dF.cpu().numpy() - F) <= TOL_F * (Fabs + 1e-3 * Fabs.max())).all()
+    dq2 = dev(q)
+    ctx.alegb_step(dq2, 0.0, cfg["dt"], 2)
+    torch.cuda.synchronize()
+    assert torch.isfinite(dq2).all().item()
     ctx.close()
 
 

@@ -101,14 +101,25 @@ def simulate(NG, NS, NB, CW, WPG, NQ, seed, every_quad):
 
 
 def _cfg(dim, N):
-    """(NG, NS, NB, CW, warps per group) as Cfg<DIM,N> of stage_pipe.cu derives them."""
-    Np = (N + 1) * (N + 2) // 2 if dim == 2 else (N + 1) * (N + 2) * (N + 3) // 6
-    NB = (Np + 7) // 8
-    if dim == 2:
-        return 6, 16, NB, 10, 1
-    if N <= 3:
-        return 2, 8, NB, 8, 2
-    return 1, 4, NB, 8, 4
+    """(NG, NS, NB, CW, warps per group) of the kernel compiled for (dim, N), read from the library itself
+    (alegb_pipe_config reports Cfg<DIM,N> of csrc/stage_pipe.cu), so that the simulation cannot drift from the kernel."""
+    from paper_2607_00199_b200 import binding
+    c = binding.alegb_pipe_config(dim, N)
+    return c["producer_groups"], c["slots"], c["items_per_quad"], c["consumer_warps"], c["warps_per_group"]
+
+
+def test_library_reports_a_consistent_configuration():
+    from paper_2607_00199_b200 import binding
+    for dim, N in [(2, 1), (2, 4), (3, 1), (3, 3), (3, 4)]:
+        c = binding.alegb_pipe_config(dim, N)
+        Np = (N + 1) * (N + 2) // 2 if dim == 2 else (N + 1) * (N + 2) * (N + 3) // 6
+        assert c["items_per_quad"] == (Np + 7) // 8 <= c["consumer_warps"]
+        assert c["producer_groups"] * c["warps_per_group"] == c["producer_warps"]
+        assert c["slots"] >= c["producer_groups"]            # a group's wait on `empty` is at most one phase off
+        assert c["smem_bytes"] <= 227 * 1024
+    with pytest.raises(binding.AlegbError) as e:
+        binding.alegb_pipe_config(3, 5)
+    assert e.value.status == binding.UNSUPPORTED
 
 
 @pytest.mark.parametrize("dim,N", [(2, 1), (2, 2), (2, 3), (2, 4), (2, 5), (3, 1), (3, 2), (3, 3), (3, 4)])

@@ -140,13 +140,15 @@ def airfoil_ogrid(ntheta=300, nr=100, R=20.0, pml_width=2.0, sigma_max=10.0, thi
     return X0, EToV, EToB, pml_sigma, centre
 
 
-def _inside_body(p, length=1.0, half_height=0.1, half_width=0.06):
-    """Ellipsoid of length 1 with the nose at x = 0 (config 5 stand-in for the fish body)."""
+def _inside_body(p, length=1.0, half_height=0.14, half_width=0.10):
+    """Ellipsoid of length 1 with the nose at x = 0 (config 5 stand-in for the fish body); the
+    default half-axes are the maxima of the paper's profiles R(x), r(x) (eq. 22): 0.14 L and ~0.10 L.  A thinner body
+    (round 1 used 0.10 / 0.06) contains no hex centre of the full-size 0.12-wide grid: the wall would vanish."""
     return ((p[..., 0] - 0.5 * length) / (0.5 * length)) ** 2 + (p[..., 1] / half_height) ** 2 + (p[..., 2] / half_width) ** 2 < 1.0
 
 
 def swimmer_box(nx=100, ny=50, nz=50, lo=(-4.0, -3.0, -3.0), hi=(8.0, 3.0, 3.0), pml_width=0.5, sigma_max=10.0,
-                half_height=0.1, half_width=0.06):
+                half_height=0.14, half_width=0.10):
     """Box of nx*ny*nz hexes x 6 Kuhn tets with the hexes whose centre lies inside the ellipsoidal body removed
     (stair-step body surface: no mesher is available; DESIGN.md input recipe, config 5).
 
