@@ -7,11 +7,17 @@ A "step" is one SARK4 time step = 4 stages, each stage = vertex motion + geometr
 relaxation / surface / SARK-update kernel (all rows of SURVEY.md 8(a)) over the whole synthetic mesh.
 Metric: GDOF-stage updates/s = K_elements * Np * Nfields * 4 * steps / time.  One JSON line on stdout (rank 0).
 
-  value        device-resident state, CUDA-event timing, max over ranks
+  value        device-resident state, CUDA-event timing of exactly --steps steps, max over ranks; the timed region is
+               repeated --repeats times (default 5) and the MEDIAN is reported (min / max beside it)
   e2e          the same steps through alegb_step_host: pinned host state -> device -> step -> host, every step
+               (plus a second figure with --steps steps per host round trip)
   roofline     the fused stage kernel: algorithmic flops (or bytes) per launch / its mean duration, measured live
                with CUDA events bracketing every launch on its stream (alegb_profile_enable)
-  cpu_baseline the oracle (oracle/, numpy, as it stands) on a bounded sample of the same workload
+  clocks       SM clock and throttle reasons polled through NVML in this process DURING the timed regions
+  per_config   the other BASELINE.json workloads (1, 2, 3, 5): value, ms per step, stage-kernel time, both roofline
+               fractions -- a driver-side record of every number DESIGN.md quotes
+  cpu_baseline the oracle (oracle/, numpy, as it stands) on a bounded sample of the same workload, one independent
+               replica per host core
   --impl reference   times the oracle alone (rank 0 only)
 
 Multi-GPU: the path is specified for one GPU (north_star: no sharding, no collectives) -> N independent replicas,
@@ -22,7 +28,7 @@ import json
 import os
 import subprocess
 import sys
-import tempfile
+import threading
 import time
 
 import numpy as np
@@ -33,15 +39,18 @@ if ROOT not in sys.path:
 
 METRIC = "GDOF-stage updates/s (nodes x fields x RK stages)"
 UNIT = "GDOF-stage/s"
-# fp64 pipe peak of one B200: 148 SMs x 64 fp64 FMA lanes per SM and clock x 2 flop x 1.965 GHz (the
-# DFMA/DMMA microbenchmark profiles/r1_fp64_peak.md measured 37.1 TFLOP/s, both instruction kinds share the pipe)
+# fp64 pipe peak of one B200: 148 SMs x 64 fp64 FMA lanes per SM and clock x 2 flop x 1.965 GHz.  MEASURED_PEAKS.json
+# holds no fp64 figure and the profiling guide no fp64 nominal, so this is DERIVED from the guide's unit count and
+# clock; the DFMA/DMMA microbenchmark of round 1 (profiles/r1_fp64_peak.md) measured 37.1 TFLOP/s with DMMA, and both
+# instruction kinds share the datapath.
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 HBM_FALLBACK_GBS = 6650.0
 ALGO_BYTES_PER_DOF_STAGE = 38.0          # 152 B per DOF-step
 POINTWISE_FLOP_PER_DOF_STAGE = 50.0
-# dram__bytes_read.sum + dram__bytes_write.sum of the stage kernel per launch from the committed `ncu --set full`
-# capture (mean over the four stages of a step: 1.79 / 2.93 / 3.48 / 1.82 GB), profiles/r1_v8_pipe_stage_kernel.md
-NCU_DRAM_BYTES_PER_LAUNCH = {4: 2.505e9}
+# dram__bytes_read.sum + dram__bytes_write.sum of the stage kernel per launch from committed `ncu --set full` captures
+# (mean over the stages of a step); configurations without a capture report no traffic figure.
+NCU_DRAM_BYTES_PER_LAUNCH = {4: (2.505e9, "profiles/r1_v8_pipe_stage_kernel.md")}
+DIM_N = {1: (2, 3), 2: (2, 4), 3: (2, 4), 4: (3, 4), 5: (3, 3)}
 
 
 def algorithmic_flop_per_dof_stage(dim, Np, Nfp):
@@ -60,7 +69,7 @@ def measured_peaks():
     return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
 
 
-def make_config(index, lam, full=True, sample=False):
+def make_config(index, lam, sample=False):
     from workloads import configs
     if sample:   # bounded sample of the same recipe for the CPU oracle
         small = {1: dict(n=8), 2: dict(n=16), 3: dict(ntheta=48, nr=16), 4: dict(n=8), 5: dict(nx=16, ny=8, nz=8)}[index]
@@ -69,57 +78,95 @@ def make_config(index, lam, full=True, sample=False):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
-    FIELDS = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    """SM clock and clock-event (throttle) reasons of one GPU, polled through NVML from a thread of this process
+    every few milliseconds; only samples taken between begin() and end() -- the timed regions -- are kept
+    (B200_PROFILING.md: clocks DURING the timed region).  Falls back to one `nvidia-smi` query per poll."""
+    REASONS = (("hw_slowdown", "nvmlClocksEventReasonHwSlowdown", 0x8), ("hw_thermal_slowdown", "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+               ("sw_thermal_slowdown", "nvmlClocksEventReasonSwThermalSlowdown", 0x20), ("sw_power_cap", "nvmlClocksEventReasonSwPowerCap", 0x4),
+               ("hw_power_brake_slowdown", "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80))
 
-    def __init__(self, gpu_index):
-        self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
-        self.proc = None
+    def __init__(self, gpu_index, period_s=0.004):
+        self.period, self.samples, self.reasons, self.active, self.stop_flag = period_s, [], set(), False, False
+        self.sm_max, self.how, self.nvml, self.handle = None, None, None, None
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.FIELDS,
-                                          "--format=csv,noheader,nounits", "-lms", "20"], stdout=self.tmp,
-                                         stderr=subprocess.DEVNULL)
+            import pynvml
+            pynvml.nvmlInit()
+            # torch's device order follows CUDA_VISIBLE_DEVICES; NVML's does not
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = gpu_index
+            if vis:
+                ids = [v.strip() for v in vis.split(",") if v.strip()]
+                if gpu_index < len(ids) and ids[gpu_index].isdigit():
+                    phys = int(ids[gpu_index])
+            self.handle = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(self.handle, pynvml.NVML_CLOCK_SM))
+            self.nvml, self.how = pynvml, "NVML in-process, %.0f ms period" % (period_s * 1e3)
         except Exception:
-            self.proc = None
+            self.how = "nvidia-smi query per poll"
+        self.gpu_index = gpu_index
+        self.thread = threading.Thread(target=self._run, daemon=True)
+        self.thread.start()
+
+    def _poll(self):
+        if self.nvml is not None:
+            n = self.nvml
+            sm = float(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM))
+            try:
+                mask = int(n.nvmlDeviceGetCurrentClocksEventReasons(self.handle))
+            except Exception:
+                mask = int(n.nvmlDeviceGetCurrentClocksThrottleReasons(self.handle))
+            return sm, [name for name, attr, bit in self.REASONS if mask & getattr(n, attr, bit)]
+        out = subprocess.run(["nvidia-smi", "-i", str(self.gpu_index), "--query-gpu=clocks.sm,clocks.max.sm,"
+                              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+                              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap",
+                              "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=10).stdout
+        r = [x.strip() for x in out.strip().splitlines()[0].split(",")]
+        self.sm_max = float(r[1])
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        return float(r[0]), [n for n, v in zip(names, r[2:6]) if v.lower().startswith("active")]
+
+    def _run(self):
+        while not self.stop_flag:
+            if self.active:
+                try:
+                    sm, reasons = self._poll()
+                    if self.active:
+                        self.samples.append(sm)
+                        self.reasons.update(reasons)
+                except Exception:
+                    pass
+            time.sleep(self.period)
+
+    def begin(self):
+        self.active = True
+
+    def end(self):
+        self.active = False
 
     def stop(self):
-        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        if self.proc is not None:
-            self.proc.terminate()
-            try:
-                self.proc.wait(timeout=5)
-            except Exception:
-                self.proc.kill()
-        try:
-            self.tmp.flush()
-            rows = [l.strip().split(",") for l in open(self.tmp.name) if l.strip()]
-            sm = [float(r[0]) for r in rows if len(r) >= 6]
-            if sm:
-                out["sm_mhz"] = float(np.median(sm))
-                out["sm_max_mhz"] = float(rows[0][1])
-                out["samples"] = len(sm)
-                names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-                for i, n in enumerate(names):
-                    if any(r[2 + i].strip().lower().startswith("active") for r in rows if len(r) >= 6):
-                        out["reasons"].append(n)
-        except Exception:
-            pass
-        finally:
-            try:
-                os.unlink(self.tmp.name)
-            except Exception:
-                pass
-        return out
+        self.stop_flag = True
+        self.thread.join(timeout=5)
+        s = self.samples
+        return {"sm_mhz": float(np.median(s)) if s else None, "sm_min_mhz": float(min(s)) if s else None,
+                "sm_max_mhz": self.sm_max, "reasons": sorted(self.reasons), "samples": len(s), "how": self.how,
+                "when": "inside the timed regions only"}
 
 
-def time_oracle(index, steps, warmup):
-    """The oracle as it stands on a bounded sample of workload `index`; returns (GDOF-stage/s, cores, description)."""
+# ------------------------------------------------------------------------------------------------- the oracle, timed
+def _oracle_replica(args):
+    """One replica of the oracle on the bounded sample (runs in a worker process, one BLAS thread)."""
+    index, steps, warmup = args
+    for v in ("OMP_NUM_THREADS", "OPENBLAS_NUM_THREADS", "MKL_NUM_THREADS"):
+        os.environ[v] = "1"
+    try:
+        from threadpoolctl import threadpool_limits
+        threadpool_limits(1)
+    except Exception:
+        pass
     from oracle import sark
     from oracle.operators import ReferenceElement
     from oracle.rhs import Problem
-    from workloads import configs
-    dim, N = {1: (2, 3), 2: (2, 4), 3: (2, 4), 4: (3, 4), 5: (3, 3)}[index]
+    dim, N = DIM_N[index]
     ref = ReferenceElement(dim, N)
     cfg = make_config(index, ref.lam, sample=True)
     P = Problem(dim, N, cfg["X0"], cfg["EToV"], cfg.get("vertex_equiv"), cfg.get("EToB"), cfg.get("pml_sigma"),
@@ -129,16 +176,31 @@ def time_oracle(index, steps, warmup):
     for n in range(warmup):
         stages, aux = sark.step_debug(P, q, n * dt, dt, aux)
         q = stages[-1]
-    w0, c0 = time.perf_counter(), time.process_time()
+    w0 = time.perf_counter()
     for n in range(steps):
         stages, aux = sark.step_debug(P, q, (warmup + n) * dt, dt, aux)
         q = stages[-1]
-    wall, cpu = time.perf_counter() - w0, time.process_time() - c0
-    dof = cfg["K"] * cfg["Np"] * cfg["Nf"]
-    cores = max(1, int(round(cpu / max(wall, 1e-9))))
-    desc = "%s recipe shrunk to K=%d elements (N=%d, %d fields), %d SARK4 steps (%d stages)" % (
-        cfg["name"], cfg["K"], N, cfg["Nf"], steps, 4 * steps)
-    return dof * 4 * steps / wall / 1e9, cores, desc, wall / max(steps, 1) * 1e3, cfg
+    wall = time.perf_counter() - w0
+    return wall, cfg["K"] * cfg["Np"] * cfg["Nf"], cfg["K"], cfg["name"], N, cfg["Nf"], bool(np.isfinite(q).all())
+
+
+def time_oracle(index, steps, warmup, cores=None):
+    """The oracle as it stands (never tuned for this) on a bounded sample of workload `index`: one independent replica
+    of the sample per host core, all started together; value = replicas x DOF x 4 x steps / slowest replica.
+    Returns (GDOF-stage/s, cores used, description, ms per step of the slowest replica)."""
+    import multiprocessing as mp
+    cores = cores or int(os.environ.get("ALEGB_BENCH_CORES", "0")) or os.cpu_count() or 1
+    if cores == 1:
+        results = [_oracle_replica((index, steps, warmup))]
+    else:
+        with mp.get_context("spawn").Pool(cores) as pool:
+            results = pool.map(_oracle_replica, [(index, steps, warmup)] * cores, chunksize=1)
+    wall = max(r[0] for r in results)
+    dof, K, name, N, Nf = results[0][1:6]
+    assert all(r[6] for r in results)
+    desc = ("%s recipe shrunk to K=%d elements (N=%d, %d fields), %d SARK4 steps (%d stages), %d independent replicas "
+            "(one per host core, numpy single-threaded each)" % (name, K, N, Nf, steps, 4 * steps, cores))
+    return cores * dof * 4 * steps / wall / 1e9, cores, desc, wall / max(steps, 1) * 1e3
 
 
 def max_over_ranks(x, world, device):
@@ -160,7 +222,7 @@ def job_throughput(dof_per_rank, steps, world, elapsed_ms):
 def run_reference(args, rank):
     if rank != 0:
         return
-    value, cores, desc, ms, cfg = time_oracle(args.config, args.steps, args.warmup)
+    value, cores, desc, ms = time_oracle(args.config, args.steps, args.warmup)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -180,11 +242,95 @@ def workload_name(index):
             5: "configs[4] 3D carangiform swimmer stand-in: ~1.5M tetrahedra, N=3, wall + far field + PML shell"}[index]
 
 
+# ------------------------------------------------------------------------------------------------- the CUDA path, timed
+def measure(index, args, B, torch, local_rank, world, barrier, sampler, repeats, steps, warmup):
+    """Times `repeats` regions of exactly `steps` SARK4 steps of workload `index` (state resident in HBM) and the fused
+    stage kernel inside them.  Returns a dict; elapsed times are this rank's (the caller takes the max over ranks)."""
+    dim, N = DIM_N[index]
+    probe = B.Context(dim, N, -1)
+    lam = probe.alegb_get_reference()["lam"]     # node coordinates for the initial state (input generation only)
+    probe.close()
+    cfg = make_config(index, lam)
+    ctx = B.context_from_config(cfg, local_rank)
+    ctx.alegb_set_kernel(args.kernel)
+    if args.no_overlap:
+        ctx.alegb_set_geometry_overlap(False)
+    if args.relax == "cubature":
+        ctx.alegb_set_relaxation(B.RELAX_CUBATURE)
+    if args.coords == "rk":
+        ctx.alegb_set_coordinate_mode(B.COORDS_RK, 0.0)
+    K, Np, Nf, Nfp = cfg["K"], cfg["Np"], cfg["Nf"], ctx.Nfp
+    dof, dt = K * Np * Nf, cfg["dt"]
+    q = torch.from_numpy(cfg["q0"]).cuda()
+    state_bytes = q.numel() * 8
+    ctx.alegb_step(q, 0.0, dt, warmup)
+    barrier()
+    # Large states (the throughput configuration): the library brackets every stage-kernel launch of the timed regions
+    # with events (direct launches).  Small, L2-resident states are launch-bound: the timed regions replay the
+    # captured step graph (alegb_set_graph) and the stage kernel is timed in a second, direct pass of the same steps.
+    graph_timed = state_bytes < 200e6
+    ctx.alegb_profile_enable(not graph_timed)
+    times, launches = [], 0
+    for r in range(repeats):
+        n0 = ctx.alegb_launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        if sampler:
+            sampler.begin()
+        e0.record()
+        ctx.alegb_step(q, (warmup + r * steps) * dt, dt, steps)
+        e1.record()
+        barrier()
+        if sampler:
+            sampler.end()
+        times.append(e0.elapsed_time(e1))
+        launches = ctx.alegb_launch_count() - n0
+    if graph_timed:
+        ctx.alegb_profile_enable(True)
+        ctx.alegb_step(q.clone(), warmup * dt, dt, steps)
+    nprof, prof_ms = ctx.alegb_profile_read()
+    ctx.alegb_profile_enable(False)
+    finite = bool(torch.isfinite(q).all().item())
+    kern_ms = prof_ms / max(nprof, 1)
+    # share of the step: stage-kernel time per step / step time (both from the same kind of launches where possible)
+    # (graph-replayed regions: the stage kernel is timed in a separate direct-launch pass whose launches do not
+    #  overlap the a1/a2 branch the same way, so a share of the replayed step is not defined)
+    share = None if graph_timed else (prof_ms / max(nprof, 1) * 4) / (float(np.median(times)) / steps)
+    return dict(cfg=cfg, ctx=ctx, q=q, dim=dim, N=N, K=K, Np=Np, Nf=Nf, Nfp=Nfp, dof=dof, dt=dt, state_bytes=state_bytes,
+                times=times, launches=launches, kern_ms=kern_ms, nprof=nprof, share=share, graph_timed=graph_timed,
+                finite=finite)
+
+
+def rooflines(m, index, kernel):
+    hbm_peak, hbm_src = measured_peaks()
+    flop_per_dof = algorithmic_flop_per_dof_stage(m["dim"], m["Np"], m["Nfp"])
+    tf = m["dof"] * flop_per_dof / (m["kern_ms"] * 1e-3) / 1e12
+    gbs = m["dof"] * ALGO_BYTES_PER_DOF_STAGE / (m["kern_ms"] * 1e-3) / 1e9
+    alu = {"bound": "alu", "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": tf / FP64_PEAK_TFLOPS,
+           "traffic": None, "peak_source": "derived: 148 SM x 64 fp64 FMA/clk x 2 x 1.965 GHz (no fp64 figure in "
+           "MEASURED_PEAKS.json; DMMA microbenchmark 37.1, profiles/r1_fp64_peak.md)",
+           "algorithmic_flop_per_dof_stage": flop_per_dof}
+    hbm = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak, "traffic": None,
+           "peak_source": hbm_src, "algorithmic_bytes_per_dof_stage": ALGO_BYTES_PER_DOF_STAGE}
+    first, other = (alu, hbm) if alu["frac"] >= hbm["frac"] else (hbm, alu)
+    first = dict(first)
+    if kernel == 0 and index in NCU_DRAM_BYTES_PER_LAUNCH:
+        first["traffic"], src = NCU_DRAM_BYTES_PER_LAUNCH[index]
+        first["traffic_unit"] = "bytes per launch (ncu dram read+write, %s)" % src
+        first["algorithmic_bytes_per_launch"] = m["dof"] * ALGO_BYTES_PER_DOF_STAGE
+    first.update({"kernel": "alegb stage kernel (fused volume+relaxation+surface+SARK update)",
+                  "kernel_ms": m["kern_ms"], "kernel_launches_timed": m["nprof"], "kernel_share_of_step": m["share"],
+                  "kernel_timed_in": "second pass, direct launches (timed regions replay the step graph)"
+                  if m["graph_timed"] else "timed regions", "other_roof": other})
+    return first
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--repeats", type=int, default=5, help="timed regions of --steps steps each; the median is reported")
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5],
                     help="BASELINE.json workload (1-based); 4 = the 3D N=4 throughput configuration")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
@@ -197,8 +343,10 @@ def main():
     ap.add_argument("--no-overlap", action="store_true", help="a1/a2 of the next stage in order instead of beside the stage kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (workloads 1, 2, 3, 5)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+    args.repeats = max(args.repeats, 1)
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -216,57 +364,17 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     from paper_2607_00199_b200 import binding as B
 
-    dim, N = {1: (2, 3), 2: (2, 4), 3: (2, 4), 4: (3, 4), 5: (3, 3)}[args.config]
-    probe = B.Context(dim, N, -1)
-    lam = probe.alegb_get_reference()["lam"]     # node coordinates for the initial state (input generation only)
-    probe.close()
-    cfg = make_config(args.config, lam)
-    ctx = B.context_from_config(cfg, local_rank)
-    ctx.alegb_set_kernel(args.kernel)
-    if args.no_overlap:
-        ctx.alegb_set_geometry_overlap(False)
-    if args.relax == "cubature":
-        ctx.alegb_set_relaxation(B.RELAX_CUBATURE)
-    if args.coords == "rk":
-        ctx.alegb_set_coordinate_mode(B.COORDS_RK, 0.0)
-    K, Np, Nf, Nfp = cfg["K"], cfg["Np"], cfg["Nf"], ctx.Nfp
-    dof = K * Np * Nf
-    dt = cfg["dt"]
-    q = torch.from_numpy(cfg["q0"]).cuda()
-    state_bytes = q.numel() * 8
-
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident timing
-    ctx.alegb_step(q, 0.0, dt, args.warmup)
-    barrier()
-    sampler = ClockSampler(local_rank) if rank == 0 else None
-    # Large states (the throughput configuration): the library brackets every stage-kernel launch of the timed region
-    # with events (direct launches).  Small, L2-resident states are launch-bound: the timed region replays the
-    # captured step graph (alegb_set_graph) and the stage kernel is timed in a second, direct pass of the same steps.
-    graph_timed = state_bytes < 200e6
-    ctx.alegb_profile_enable(not graph_timed)
-    n0 = ctx.alegb_launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record()
-    ctx.alegb_step(q, args.warmup * dt, dt, args.steps)
-    e1.record()
-    barrier()
-    elapsed_ms = e0.elapsed_time(e1)
-    launches = ctx.alegb_launch_count() - n0
-    if graph_timed:
-        ctx.alegb_profile_enable(True)
-        ctx.alegb_step(q.clone(), args.warmup * dt, dt, args.steps)
-    nprof, prof_ms = ctx.alegb_profile_read()
-    ctx.alegb_profile_enable(False)
-    clocks = sampler.stop() if sampler else None
-    elapsed_ms = max_over_ranks(elapsed_ms, world, "cuda")
-    finite = bool(torch.isfinite(q).all().item())
-    value = job_throughput(dof, args.steps, world, elapsed_ms)
+    sampler = ClockSampler(local_rank) if rank == 0 else None      # started before the warm-up
+    m = measure(args.config, args, B, torch, local_rank, world, barrier, sampler, args.repeats, args.steps, args.warmup)
+    times = [max_over_ranks(t, world, "cuda") for t in m["times"]]
+    elapsed_ms = float(np.median(times))
+    value = job_throughput(m["dof"], args.steps, world, elapsed_ms)
+    ctx, cfg, dof, dt, state_bytes = m["ctx"], m["cfg"], m["dof"], m["dt"], m["state_bytes"]
 
     # ---- end to end through the host-buffer entry point (pinned host state, H2D + step + D2H every step)
     e2e = None
@@ -275,61 +383,83 @@ def main():
         ctx.alegb_step_host(hq, 0.0, dt, 1)
         barrier()
         nsteps_e2e = max(3, min(args.steps, 10))
+        if sampler:
+            sampler.begin()
         t0 = time.perf_counter()
         for n in range(nsteps_e2e):
             ctx.alegb_step_host(hq, (1 + n) * dt, dt, 1)
         torch.cuda.synchronize()
-        el = time.perf_counter() - t0
-        el = max_over_ranks(el, world, "cuda")
+        el = max_over_ranks(time.perf_counter() - t0, world, "cuda")
+        # second figure: one host round trip per --steps steps (the state crosses PCIe twice per CALL, not per step)
+        t0 = time.perf_counter()
+        ctx.alegb_step_host(hq, (1 + nsteps_e2e) * dt, dt, args.steps)
+        torch.cuda.synchronize()
+        el_b = max_over_ranks(time.perf_counter() - t0, world, "cuda")
+        if sampler:
+            sampler.end()
         e2e = {"value": job_throughput(dof, nsteps_e2e, world, el * 1e3), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
-               "d2h_bytes_per_step": state_bytes, "steps": nsteps_e2e, "api": "alegb_step_host (pinned host buffer)"}
+               "d2h_bytes_per_step": state_bytes, "steps": nsteps_e2e, "api": "alegb_step_host (pinned host buffer), one step per call",
+               "batched": {"value": job_throughput(dof, args.steps, world, el_b * 1e3), "unit": UNIT,
+                           "steps_per_call": args.steps, "h2d_bytes_per_step": state_bytes / args.steps,
+                           "d2h_bytes_per_step": state_bytes / args.steps}}
+    ctx.close()
+    del m["q"]
+    torch.cuda.empty_cache()
+
+    # ---- the other workloads (rank 0's GPU only, after the headline numbers; a few seconds each)
+    per_config = None
+    if not args.no_per_config and world == 1:
+        per_config = {}
+        for idx in (1, 2, 3, 5):
+            if idx == args.config:
+                continue
+            try:
+                st = 50 if idx in (1, 2) else (20 if idx == 3 else 5)
+                mm = measure(idx, args, B, torch, local_rank, 1, barrier, sampler, 3, st, 3)
+                el = float(np.median(mm["times"]))
+                rf = rooflines(mm, idx, args.kernel)
+                per_config[str(idx)] = {
+                    "workload": workload_name(idx), "K": mm["K"], "dof": mm["dof"], "steps": st, "repeats": 3,
+                    "value": job_throughput(mm["dof"], st, 1, el), "unit": UNIT, "ms_per_step": el / st,
+                    "stage_kernel_ms": mm["kern_ms"], "stage_kernel_share_of_step": mm["share"],
+                    "frac_fp64": (rf if rf["bound"] == "alu" else rf["other_roof"])["frac"],
+                    "frac_hbm": (rf if rf["bound"] == "hbm" else rf["other_roof"])["frac"],
+                    "gpu_launches_per_region": int(mm["launches"]), "state_finite": mm["finite"],
+                    "launch": "one CUDA graph per step" if mm["graph_timed"] else "direct launches"}
+                mm["ctx"].close()
+                del mm
+                torch.cuda.empty_cache()
+            except Exception as e:      # a failed side measurement must not lose the headline line
+                per_config[str(idx)] = {"error": repr(e)[:300]}
+    clocks = sampler.stop() if sampler else None
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (the fused stage kernel)
-    hbm_peak, hbm_src = measured_peaks()
-    kern_ms = prof_ms / max(nprof, 1)
-    flop_per_dof = algorithmic_flop_per_dof_stage(dim, Np, Nfp)
-    tf = dof * flop_per_dof / (kern_ms * 1e-3) / 1e12
-    gbs = dof * ALGO_BYTES_PER_DOF_STAGE / (kern_ms * 1e-3) / 1e9
-    alu = {"bound": "alu", "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": tf / FP64_PEAK_TFLOPS,
-           "traffic": None, "peak_source": "derived: 148 SM x 64 fp64 FMA/clk x 2 x 1.965 GHz (DESIGN.md)",
-           "algorithmic_flop_per_dof_stage": flop_per_dof}
-    hbm = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak, "traffic": None,
-           "peak_source": hbm_src, "algorithmic_bytes_per_dof_stage": ALGO_BYTES_PER_DOF_STAGE}
-    roofline, other = (alu, hbm) if alu["frac"] >= hbm["frac"] else (hbm, alu)
-    roofline = dict(roofline)
-    if args.kernel == 0:
-        roofline["traffic"] = NCU_DRAM_BYTES_PER_LAUNCH.get(args.config)
-        roofline["traffic_unit"] = "bytes per launch (ncu dram read+write, profiles/r1_v8_pipe_stage_kernel.md)"
-        roofline["algorithmic_bytes_per_launch"] = dof * ALGO_BYTES_PER_DOF_STAGE
-    roofline.update({"kernel": "alegb stage kernel (fused volume+relaxation+surface+SARK update)",
-                     "kernel_ms": kern_ms, "kernel_launches_timed": nprof,
-                     "kernel_share_of_step": prof_ms / elapsed_ms if elapsed_ms > 0 else None,
-                     "kernel_timed_in": "second pass, direct launches (timed region replays the step graph)"
-                     if graph_timed else "timed region",
-                     "other_roof": other})
-
+    roofline = rooflines(m, args.config, args.kernel)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(args.config), "K": K, "N": N, "Np": Np, "Nfields": Nf, "dof": dof,
-                       "dt": dt, "parallelism": "replicas x%d (north_star: one GPU, no sharding)" % world,
+            "repeats": {"n": args.repeats, "statistic": "median", "ms_per_step_min": min(times) / args.steps,
+                        "ms_per_step_max": max(times) / args.steps,
+                        "value_min": job_throughput(dof, args.steps, world, max(times)),
+                        "value_max": job_throughput(dof, args.steps, world, min(times))},
+            "config": {"workload": workload_name(args.config), "K": m["K"], "N": m["N"], "Np": m["Np"], "Nfields": m["Nf"],
+                       "dof": dof, "dt": dt, "parallelism": "replicas x%d (north_star: one GPU, no sharding)" % world,
                        "l2": "state arrays are %.0f MB each (> 126 MB L2), no flush needed" % (state_bytes / 1e6)
                        if state_bytes > 200e6 else "state is L2-resident (%.1f MB); launch-latency bound" % (state_bytes / 1e6),
-                       "state_finite": finite, "kernel": args.kernel, "relax": args.relax, "coords": args.coords,
-                       "launch": "one CUDA graph per step" if graph_timed and args.steps >= 2 else "direct launches"},
-            "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
-
+                       "state_finite": m["finite"], "kernel": args.kernel, "relax": args.relax, "coords": args.coords,
+                       "launch": "one CUDA graph per step" if m["graph_timed"] and args.steps >= 2 else "direct launches"},
+            "e2e": e2e, "gpu_launches": int(m["launches"]), "clocks": clocks, "roofline": roofline}
+    if per_config is not None:
+        line["per_config"] = per_config
     if not args.no_cpu_baseline:
-        v, cores, desc, _, _ = time_oracle(args.config, 6 if args.config in (4, 5) else 20, 1)
+        v, cores, desc, _ = time_oracle(args.config, 6 if args.config in (4, 5) else 20, 1)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
                                 "host_cores_available": os.cpu_count()}
     print(json.dumps(line), flush=True)
-    ctx.close()
     if world > 1:
         dist.destroy_process_group()
 
