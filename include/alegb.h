@@ -63,7 +63,8 @@ typedef enum {
  *   CARANGIFORM    PAPER.md:L339-365 (reading R13): lateral displacement along `axis`
  *                  (a0+a1 x~+a2 x~^2) sin(k X - omega t) B(d_eff) S(t);
  *                  params = [a0, a1, a2, k, omega, R_rigid, beta, T_ramp, axis, Bcut]
- *   USER           positions/velocities supplied by alegb_set_motion_user (device arrays, constant in time)
+ *   USER           positions/velocities supplied by alegb_set_motion_user (constant in time) or, per RK stage, by
+ *                  alegb_set_motion_user_stages
  */
 typedef enum {
   ALEGB_MOTION_NONE = 0,
@@ -79,8 +80,8 @@ typedef enum {
  *   RK           the coordinates are "advanced in time using the same Runge-Kutta integration scheme employed for the
  *                primary solver" (L152; L233 dx/dt = v_G): classic RK4 on dx/dt = v(X0, t) with the law's vertex
  *                velocity; stage i sees x^(i) = x_n + dt a_{i,i-1} v(t_{i-1}) and the velocity v(t_i), and the step
- *                ends with x_{n+1} = x_n + dt sum_j b_j v(t_j).  Motion kind USER: the supplied velocity, constant in
- *                time.  (SURVEY 8(f) NEXT-2.)  alegb_rhs and alegb_geometry always evaluate the closed form. */
+ *                ends with x_{n+1} = x_n + dt sum_j b_j v(t_j).  Motion kind USER: the supplied stage velocities
+ *                (alegb_set_motion_user_stages; alegb_set_motion_user: one velocity for all stages).  (SURVEY 8(f) NEXT-2.)  alegb_rhs and alegb_geometry always evaluate the closed form. */
 typedef enum { ALEGB_COORDS_CLOSED_FORM = 0, ALEGB_COORDS_RK = 1 } alegb_coord_mode;
 
 /* How the nonlinear relaxation N~(q) enters F.
@@ -115,8 +116,23 @@ int alegb_set_params(alegb_ctx* ctx, double RT, double tau, const double* q_inf)
 /* Prescribed motion law (see alegb_motion_kind); params is a HOST array, copied. */
 int alegb_set_motion(alegb_ctx* ctx, int kind, const double* params, int nparams);
 /* kind USER: DEVICE arrays [Nverts*dim] of vertex positions and velocities, copied device-to-device on the
- * default stream and used for every subsequent evaluation until the motion is set again. */
+ * default stream and used for every subsequent evaluation (all four stages of every step: a velocity constant in
+ * time) until the motion is set again.  Synchronises the default stream. */
 int alegb_set_motion_user(alegb_ctx* ctx, const double* d_xv, const double* d_vv);
+/* kind USER with data that change from stage to stage ("During each Runge-Kutta stage, we evaluate the
+ * explicit, continuous velocity field v_G and subsequently update the spatial coordinates"; L391 fluid-structure
+ * outlook): DEVICE arrays [4][Nverts*dim], entry i belongs to RK stage i of the NEXT step
+ * (stage times t_n + (0, 1/2, 1/2, 1) dt); copied.  Every following alegb_step / alegb_step_debug step uses the same
+ * four entries, so a caller whose velocities change in time calls this before each single step.
+ *   coordinate mode CLOSED_FORM: stage i sees the positions d_xv4[i] and the velocities d_vv4[i].
+ *   coordinate mode RK: d_xv4 is ignored except for entry 0 on the first call (the starting positions, see
+ *     alegb_set_coordinate_mode) and may be NULL afterwards; the library integrates the positions with the classic
+ *     RK4 of the solver and the caller's stage velocities k_i = d_vv4[i-1]:
+ *       x^(1) = x_n + dt/2 k_1,  x^(2) = x_n + dt/2 k_2,  x^(3) = x_n + dt k_3,  x_{n+1} = x_n + dt/6 (k_1+2k_2+2k_3+k_4),
+ *     stage i of the fields sees x^(i) and k_{i+1}.
+ * alegb_rhs, alegb_geometry and alegb_wall_forces (one evaluation, no stage) use entry 0.
+ * Errors: INVALID_ARG (d_vv4 NULL; d_xv4 NULL before any positions were supplied), NOT_READY, CUDA_ERROR. */
+int alegb_set_motion_user_stages(alegb_ctx* ctx, const double* d_xv4, const double* d_vv4);
 
 /* Select the relaxation mode for alegb_rhs / alegb_step (every stage kernel honours it).  CUBATURE builds the rule
  * and I, P on the host, uploads them and allocates R[K][dim(dim+1)/2][Np] (part of alegb_workspace_bytes).

@@ -32,12 +32,19 @@ def velocity(problem, t):
     return _motion.vertices(problem.motion_kind, problem.motion_params, problem.X0, t)[1]
 
 
-def stage_vertices(problem, x_n, t0, dt):
-    """The four (positions, velocities) pairs of one step, and x_{n+1}."""
-    k1 = velocity(problem, t0 + _sark.RK4_C[0] * dt)
-    k2 = velocity(problem, t0 + _sark.RK4_C[1] * dt)
-    k3 = velocity(problem, t0 + _sark.RK4_C[2] * dt)
-    k4 = velocity(problem, t0 + _sark.RK4_C[3] * dt)
+def stage_vertices(problem, x_n, t0, dt, stage_velocities=None):
+    """The four (positions, velocities) pairs of one step, and x_{n+1}.
+
+    stage_velocities: optional (k_1, k_2, k_3, k_4), vertex velocities supplied by the caller for the four stages
+    instead of the prescribed law (L152: "we evaluate the explicit, continuous velocity field v_G" at each stage; a
+    velocity that depends on the positions, as in fluid-structure coupling (L391), has k_2 != k_3)."""
+    if stage_velocities is None:
+        k1 = velocity(problem, t0 + _sark.RK4_C[0] * dt)
+        k2 = velocity(problem, t0 + _sark.RK4_C[1] * dt)
+        k3 = velocity(problem, t0 + _sark.RK4_C[2] * dt)
+        k4 = velocity(problem, t0 + _sark.RK4_C[3] * dt)
+    else:
+        k1, k2, k3, k4 = (np.asarray(k, dtype=float) for k in stage_velocities)
     x0 = x_n
     x1 = x_n + dt * _sark.RK4_A[1][0] * k1
     x2 = x_n + dt * _sark.RK4_A[2][1] * k2
@@ -46,9 +53,9 @@ def stage_vertices(problem, x_n, t0, dt):
     return [(x0, k1), (x1, k2), (x2, k3), (x3, k4)], x_next
 
 
-def step_debug(problem, q, x_n, t0, dt, aux=None):
+def step_debug(problem, q, x_n, t0, dt, aux=None, stage_velocities=None):
     """One SARK4 step on RK-integrated coordinates.  Returns (stages, aux_new, x_{n+1})."""
-    verts, x_next = stage_vertices(problem, x_n, t0, dt)
+    verts, x_next = stage_vertices(problem, x_n, t0, dt, stage_velocities)
     stages, auxn = _sark.step_debug(problem, q, t0, dt, aux, verts=verts)
     return stages, auxn, x_next
 

@@ -32,6 +32,7 @@ _SIGNATURES = {
     "alegb_set_params": (_c.c_int, [_P, _c.c_double, _c.c_double, _P]),
     "alegb_set_motion": (_c.c_int, [_P, _c.c_int, _P, _c.c_int]),
     "alegb_set_motion_user": (_c.c_int, [_P, _P, _P]),
+    "alegb_set_motion_user_stages": (_c.c_int, [_P, _P, _P]),
     "alegb_set_coordinate_mode": (_c.c_int, [_P, _c.c_int, _c.c_double]),
     "alegb_set_relaxation": (_c.c_int, [_P, _c.c_int]),
     "alegb_set_geometry_overlap": (_c.c_int, [_P, _c.c_int]),
@@ -151,6 +152,10 @@ class Context:
 
     def alegb_set_motion_user(self, d_xv, d_vv):
         self._check(_lib.alegb_set_motion_user(self._h, _dev(d_xv), _dev(d_vv)))
+
+    def alegb_set_motion_user_stages(self, d_xv4, d_vv4):
+        """d_xv4 (or None), d_vv4: CUDA tensors [4, Nverts, dim] -- the data of the four RK stages of the next step."""
+        self._check(_lib.alegb_set_motion_user_stages(self._h, _dev(d_xv4), _dev(d_vv4)))
 
     def alegb_wall_forces(self, t, d_q, tag=1, stream=None):
         """-> (F_p[dim], F_v[dim]) host arrays."""

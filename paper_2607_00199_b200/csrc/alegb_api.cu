@@ -41,7 +41,8 @@ struct alegb_ctx {
   int cub_EB = 0;                     // elements per CTA pass of cubature_relax_kernel
   double *d_It = nullptr, *d_Pt = nullptr, *d_R = nullptr;
   double *d_AI = nullptr, *d_AP = nullptr;   // I, P in DMMA A-fragment order (cubature_mma_kernel)
-  double *d_xn = nullptr, *d_user_vv = nullptr;
+  double *d_xn = nullptr;
+  double *d_user_xv = nullptr, *d_user_vv = nullptr;   // kind USER: the caller's data of the four stages, [4][Nverts*dim] each
   int32_t *d_EToV = nullptr, *d_vmapP = nullptr;
   int8_t* d_EToB = nullptr;
   double *d_vgeo = nullptr, *d_sgeo = nullptr, *d_vvel = nullptr;
@@ -112,7 +113,7 @@ void dev_free(T*& p) {
 }
 
 void free_mesh(alegb_ctx* ctx) {
-  dev_free(ctx->d_xn); dev_free(ctx->d_user_vv); ctx->coord_mode = ALEGB_COORDS_CLOSED_FORM;
+  dev_free(ctx->d_xn); dev_free(ctx->d_user_xv); dev_free(ctx->d_user_vv); ctx->coord_mode = ALEGB_COORDS_CLOSED_FORM;
   dev_free(ctx->d_R); ctx->relax_mode = ALEGB_RELAX_COLLOCATION;
   dev_free(ctx->d_X0); dev_free(ctx->d_xv); dev_free(ctx->d_vv); dev_free(ctx->d_EToV); dev_free(ctx->d_vmapP);
   dev_free(ctx->d_EToB); dev_free(ctx->d_vgeo); dev_free(ctx->d_sgeo); dev_free(ctx->d_vvel);
@@ -128,13 +129,19 @@ void free_mesh(alegb_ctx* ctx) {
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 // a1 + a2 at time t into the context's geometry arrays
-int update_geometry(alegb_ctx* ctx, double t, cudaStream_t s, const double* t_dev = nullptr) {
+// (kind USER: no a1 launch, a2 reads the caller's positions / velocities of RK stage `stage`)
+int update_geometry(alegb_ctx* ctx, double t, cudaStream_t s, const double* t_dev = nullptr, int stage = 0) {
   const int dim = ctx->ref.dim;
+  const double *xv = ctx->d_xv, *vv = ctx->d_vv;
   if (ctx->motion.kind != ALEGB_MOTION_USER) {
     CU(launch_vertex_motion(dim, ctx->Nverts, ctx->d_X0, ctx->motion, t, t_dev, ctx->d_xv, ctx->d_vv, s));
     ctx->launches++;
+  } else {
+    const size_t n = (size_t)ctx->Nverts * dim;
+    xv = ctx->d_user_xv + stage * n;
+    vv = ctx->d_user_vv + stage * n;
   }
-  CU(launch_geometry(dim, ctx->K, ctx->d_EToV, ctx->d_xv, ctx->d_vv, ctx->vg(), ctx->sg(), ctx->vvl(), s));
+  CU(launch_geometry(dim, ctx->K, ctx->d_EToV, xv, vv, ctx->vg(), ctx->sg(), ctx->vvl(), s));
   ctx->launches++;
   return ALEGB_OK;
 }
@@ -265,7 +272,7 @@ int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t
       ctx->geo_buf = j & 1;
       const double tj = t0 + cstage[j] * dt;
       return ctx->coord_mode == ALEGB_COORDS_RK ? update_geometry_rk(ctx, j, t0, dt, gs, t_dev)
-                                                 : update_geometry(ctx, tj, gs, t_dev ? t_dev + j : nullptr);
+                                                 : update_geometry(ctx, tj, gs, t_dev ? t_dev + j : nullptr, j);
     };
     (void)ti;
     int rc = ALEGB_OK;
@@ -613,21 +620,38 @@ int alegb_set_motion(alegb_ctx* ctx, int kind, const double* params, int nparams
   return ALEGB_OK;
 }
 
-int alegb_set_motion_user(alegb_ctx* ctx, const double* d_xv, const double* d_vv) {
+// kind USER: stage data [4][Nverts*dim]; `stride` = 0 replicates one array over the four stages
+static int set_user_motion(alegb_ctx* ctx, const double* d_xv, const double* d_vv, size_t stride) {
   if (!ctx) return ALEGB_INVALID_ARG;
   if (ctx->device < 0) return fail(ctx, ALEGB_CUDA_ERROR, "host-only context (no CUDA device)");
   if (!ctx->mesh_ready) return fail(ctx, ALEGB_NOT_READY, "alegb_mesh_upload has not been called");
-  if (!d_xv || !d_vv) return fail(ctx, ALEGB_INVALID_ARG, "NULL device array");
+  if (!d_vv) return fail(ctx, ALEGB_INVALID_ARG, "NULL device array");
+  if (!d_xv && !ctx->d_user_xv) return fail(ctx, ALEGB_INVALID_ARG, "positions are required the first time");
   CU(cudaSetDevice(ctx->device));
-  const size_t bytes = (size_t)ctx->Nverts * ctx->ref.dim * sizeof(double);
-  CU(cudaMemcpyAsync(ctx->d_xv, d_xv, bytes, cudaMemcpyDeviceToDevice, 0));
-  CU(cudaMemcpyAsync(ctx->d_vv, d_vv, bytes, cudaMemcpyDeviceToDevice, 0));
-  if (!ctx->d_user_vv) CU(dev_alloc(ctx, &ctx->d_user_vv, (size_t)ctx->Nverts * ctx->ref.dim));
-  CU(cudaMemcpyAsync(ctx->d_user_vv, d_vv, bytes, cudaMemcpyDeviceToDevice, 0));
+  const size_t n = (size_t)ctx->Nverts * ctx->ref.dim, bytes = n * sizeof(double);
+  if (!ctx->d_user_xv) CU(dev_alloc(ctx, &ctx->d_user_xv, 4 * n));
+  if (!ctx->d_user_vv) CU(dev_alloc(ctx, &ctx->d_user_vv, 4 * n));
+  for (int i = 0; i < 4; ++i) {
+    if (d_xv) CU(cudaMemcpyAsync(ctx->d_user_xv + i * n, d_xv + i * stride, bytes, cudaMemcpyDeviceToDevice, 0));
+    CU(cudaMemcpyAsync(ctx->d_user_vv + i * n, d_vv + i * stride, bytes, cudaMemcpyDeviceToDevice, 0));
+  }
+  // the library's "current" vertices (alegb_geometry / alegb_get_positions outputs): the first stage
+  CU(cudaMemcpyAsync(ctx->d_xv, ctx->d_user_xv, bytes, cudaMemcpyDeviceToDevice, 0));
+  CU(cudaMemcpyAsync(ctx->d_vv, ctx->d_user_vv, bytes, cudaMemcpyDeviceToDevice, 0));
   CU(cudaStreamSynchronize(0));
+  if (ctx->motion.kind != ALEGB_MOTION_USER) ctx->config_version++;   // the step graph reads the library's own buffers
   ctx->motion.kind = ALEGB_MOTION_USER;
-  ctx->config_version++;
   return ALEGB_OK;
+}
+
+int alegb_set_motion_user(alegb_ctx* ctx, const double* d_xv, const double* d_vv) {
+  if (ctx && !d_xv) return fail(ctx, ALEGB_INVALID_ARG, "NULL device array");
+  return set_user_motion(ctx, d_xv, d_vv, 0);
+}
+
+int alegb_set_motion_user_stages(alegb_ctx* ctx, const double* d_xv4, const double* d_vv4) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  return set_user_motion(ctx, d_xv4, d_vv4, (size_t)ctx->Nverts * ctx->ref.dim);
 }
 
 static int ensure_cubature(alegb_ctx* ctx) {

@@ -109,26 +109,34 @@ __global__ void vertex_rk_kernel(int64_t Nverts, const double* __restrict__ X0, 
   int64_t v = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (v >= Nverts) return;
   if (ts_dev != nullptr) { t_n = ts_dev[0]; t_h = ts_dev[1]; t_e = ts_dev[3]; dt = ts_dev[-1]; }
-  double X[DIM], xn[DIM], disp[DIM], k1[DIM], k2[DIM], k4[DIM];
+  double X[DIM], xn[DIM], disp[DIM], k1[DIM], k2[DIM], k3[DIM], k4[DIM];
 #pragma unroll
   for (int d = 0; d < DIM; ++d) { X[d] = X0[v * DIM + d]; xn[d] = x_n[v * DIM + d]; }
-  if (user_vv != nullptr) {
+  if (user_vv != nullptr) {   // kind USER: the caller's vertex velocities of the four stages, [4][Nverts][DIM]
+    const int64_t n = Nverts * DIM;
 #pragma unroll
-    for (int d = 0; d < DIM; ++d) k1[d] = k2[d] = k4[d] = user_vv[v * DIM + d];
-  } else {
+    for (int d = 0; d < DIM; ++d) {
+      k1[d] = user_vv[v * DIM + d];
+      k2[d] = user_vv[n + v * DIM + d];
+      k3[d] = user_vv[2 * n + v * DIM + d];
+      k4[d] = user_vv[3 * n + v * DIM + d];
+    }
+  } else {                    // a law v(X0, t): the two middle stages see the same velocity
     motion_law<DIM>(m, X, t_n, disp, k1);
     motion_law<DIM>(m, X, t_h, disp, k2);
     motion_law<DIM>(m, X, t_e, disp, k4);
+#pragma unroll
+    for (int d = 0; d < DIM; ++d) k3[d] = k2[d];
   }
 #pragma unroll
   for (int d = 0; d < DIM; ++d) {
     double x, w;
     if (stage == 0) { x = xn[d]; w = k1[d]; }
     else if (stage == 1) { x = fma(0.5 * dt, k1[d], xn[d]); w = k2[d]; }
-    else if (stage == 2) { x = fma(0.5 * dt, k2[d], xn[d]); w = k2[d]; }
-    else if (stage == 3) { x = fma(dt, k2[d], xn[d]); w = k4[d]; }
+    else if (stage == 2) { x = fma(0.5 * dt, k2[d], xn[d]); w = k3[d]; }
+    else if (stage == 3) { x = fma(dt, k3[d], xn[d]); w = k4[d]; }
     else {
-      x_n[v * DIM + d] = xn[d] + dt * ((1.0 / 6.0) * k1[d] + (1.0 / 3.0) * k2[d] + (1.0 / 3.0) * k2[d] + (1.0 / 6.0) * k4[d]);
+      x_n[v * DIM + d] = xn[d] + dt * ((1.0 / 6.0) * k1[d] + (1.0 / 3.0) * k2[d] + (1.0 / 3.0) * k3[d] + (1.0 / 6.0) * k4[d]);
       continue;
     }
     xv[v * DIM + d] = x;

@@ -666,3 +666,80 @@ def test_low_orders_with_many_quads_per_cta(dim, N, n, refs, B):
             for i in range(4):
                 assert rel_linf(st[i].cpu().numpy(), so[i]) <= TOL_STAGE
         ctx.close()
+
+
+# ------------------------------------------------------------------ NEXT-2, general: stage data supplied by the caller
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", ["cfg1", "cfg4"])
+def test_user_stage_data_of_the_law_equal_the_builtin_modes_bit_for_bit(name, refs, B):
+    """alegb_set_motion_user_stages fed with the law's own positions / velocities at the four stage times must give
+    the bits of the built-in law, in closed-form mode and with RK-integrated coordinates (x_n included)."""
+    ref, cfg = make_case(name, refs)
+    q = perturbed(cfg)
+    dt, t0, nsteps = cfg["dt"], 0.3, 3
+    for rk in (0, 1):
+        built = B.context_from_config(cfg)
+        user = B.context_from_config(cfg)
+        helper = B.context_from_config(cfg)                    # evaluates the law at the stage times
+        if rk:
+            built.alegb_set_coordinate_mode(B.COORDS_RK, t0)
+        qa, qb = dev(q), dev(q)
+        built.alegb_step(qa, t0, dt, nsteps)                   # three steps, through the captured graph
+        nv = cfg["X0"].shape
+        for n in range(nsteps):
+            xv4 = torch.empty((4,) + nv, dtype=torch.float64, device="cuda")
+            vv4 = torch.empty_like(xv4)
+            for i, c in enumerate((0.0, 0.5, 0.5, 1.0)):
+                helper.alegb_geometry((t0 + n * dt) + c * dt, d_xv=xv4[i], d_vv=vv4[i])
+            torch.cuda.synchronize()
+            user.alegb_set_motion_user_stages(xv4, vv4)
+            if rk and n == 0:
+                user.alegb_set_coordinate_mode(B.COORDS_RK, t0)   # x_n = the positions of entry 0
+            user.alegb_step(qb, t0 + n * dt, dt, 1)
+        torch.cuda.synchronize()
+        assert torch.equal(qa, qb)
+        if rk:
+            xa = torch.empty(nv, dtype=torch.float64, device="cuda"); xb = torch.empty_like(xa)
+            built.alegb_get_positions(xa); user.alegb_get_positions(xb)
+            torch.cuda.synchronize()
+            assert torch.equal(xa, xb)
+        built.close(); user.close(); helper.close()
+
+
+@pytest.mark.gpu
+def test_user_stage_velocities_that_depend_on_the_positions_match_oracle(refs, B):
+    """A rigid rotation of the whole (non-periodic view of the) mesh about its centre: v = Omega x (x - c) evaluated
+    by the caller at its own RK stage positions (k_2 != k_3), RK coordinate mode.  Stage states and x_{n+1} against
+    oracle/coords.py with the same four velocities; a uniform state stays uniform (GCL)."""
+    from oracle import coords
+    ref, cfg = make_case("cfg3", refs)                         # no periodic faces: a rotation is admissible
+    P = oracle_problem(cfg, ref)
+    om, cen = 20.0, np.array([0.5, 0.0])      # fast enough for k_2 - k_3 = O((om dt)^2) to be visible at the CFL step
+    rot = lambda x: om * np.stack([-(x[:, 1] - cen[1]), x[:, 0] - cen[0]], axis=1)
+    q = perturbed(cfg)
+    dt, t0 = cfg["dt"], 0.0
+    ctx = B.context_from_config(cfg)
+    x = cfg["X0"].copy()
+    dq = dev(q)
+    qo, auxo = q, None
+    for n in range(2):
+        k1 = rot(x); k2 = rot(x + 0.5 * dt * k1); k3 = rot(x + 0.5 * dt * k2); k4 = rot(x + dt * k3)
+        assert np.abs(k2 - k3).max() > 1e-9 * np.abs(k2).max()
+        ks = np.stack([k1, k2, k3, k4])
+        ctx.alegb_set_motion_user_stages(dev(np.stack([x] * 4)) if n == 0 else None, dev(ks))
+        if n == 0:
+            ctx.alegb_set_coordinate_mode(B.COORDS_RK, t0)
+        st = torch.empty((4,) + q.shape, dtype=torch.float64, device="cuda")
+        ctx.alegb_step_debug(dq, t0 + n * dt, dt, st)          # observes the stages, leaves x_n and q alone
+        ctx.alegb_pml_set(dev(auxo)) if auxo is not None else ctx.alegb_pml_reset()
+        ctx.alegb_step(dq, t0 + n * dt, dt, 1)
+        dx = torch.empty(x.shape, dtype=torch.float64, device="cuda")
+        ctx.alegb_get_positions(dx)
+        torch.cuda.synchronize()
+        so, auxo, x = coords.step_debug(P, qo, x, t0 + n * dt, dt, auxo, stage_velocities=(k1, k2, k3, k4))
+        for i in range(4):
+            assert rel_linf(st[i].cpu().numpy(), so[i]) <= TOL_STAGE
+        qo = so[-1]
+        assert rel_linf(dq.cpu().numpy(), qo) <= 2 * TOL_STAGE   # second step: each side continues from its own state
+        assert np.abs(dx.cpu().numpy() - x).max() <= 1e-14 * np.abs(x).max()
+    ctx.close()

@@ -102,3 +102,48 @@ def test_static_mesh_equals_closed_form_step(refs):
     assert np.array_equal(x1, P.X0)
     for sa, sb in zip(a, b):
         assert np.array_equal(sa, sb)
+
+
+# ------------------------------------------------------------------ caller-supplied stage velocities (NEXT-2, general)
+def test_stage_velocities_of_the_law_reproduce_the_law_bit_for_bit(refs):
+    ref = refs(2, 3)
+    cfg = configs.config1(ref.lam, n=4)
+    P = oracle_problem(cfg, ref)
+    rng = np.random.default_rng(3)
+    q = cfg["q0"] * (1.0 + 1e-3 * rng.standard_normal(cfg["q0"].shape))
+    t0, dt = 0.2, cfg["dt"]
+    ks = [motion.vertices(P.motion_kind, P.motion_params, P.X0, t0 + c * dt)[1] for c in sark.RK4_C]
+    x_n = motion.vertices(P.motion_kind, P.motion_params, P.X0, t0)[0]
+    a, _, xa = coords.step_debug(P, q, x_n, t0, dt)
+    b, _, xb = coords.step_debug(P, q, x_n, t0, dt, stage_velocities=ks)
+    assert np.array_equal(xa, xb) and all(np.array_equal(u, v) for u, v in zip(a, b))
+
+
+def test_position_dependent_velocity_rigid_rotation_is_fourth_order():
+    """dx/dt = Omega x x depends on the positions, so k_2 != k_3: the caller (here: the test, standing in for a
+    structure solver) evaluates its velocity at the stage positions it derives itself and hands the four
+    k_i over.  x_{n+1} must be the classic RK4 update (L152: "the same Runge-Kutta integration scheme"), whose
+    amplification of a rotation by angle h is the degree-4 Taylor polynomial of e^{ih} -- a closed form."""
+    class Bare:      # stage_vertices needs no Problem when the velocities are supplied
+        pass
+    om = 1.3
+    x0 = np.array([[1.0, 0.0], [0.3, -0.7], [-2.0, 0.5]])
+    rot = lambda x: om * np.stack([-x[:, 1], x[:, 0]], axis=1)
+    T = 0.9
+    errs = []
+    for n in (4, 8, 16):
+        dt, x = T / n, x0.copy()
+        for _ in range(n):
+            k1 = rot(x); k2 = rot(x + 0.5 * dt * k1); k3 = rot(x + 0.5 * dt * k2); k4 = rot(x + dt * k3)
+            verts, x_next = coords.stage_vertices(Bare(), x, 0.0, dt, stage_velocities=(k1, k2, k3, k4))
+            # the stage positions the oracle hands to the field update are the ones the velocities were evaluated at
+            assert np.allclose(verts[1][0], x + 0.5 * dt * k1, atol=1e-15) and np.allclose(verts[2][0], x + 0.5 * dt * k2, atol=1e-15)
+            assert np.allclose(verts[3][0], x + dt * k3, atol=1e-15) and np.array_equal(verts[2][1], k3)
+            z, h = x[:, 0] + 1j * x[:, 1], om * dt
+            amp = 1 + 1j * h + (1j * h) ** 2 / 2 + (1j * h) ** 3 / 6 + (1j * h) ** 4 / 24
+            assert np.allclose(x_next[:, 0] + 1j * x_next[:, 1], amp * z, rtol=0, atol=1e-14)
+            x = x_next
+        exact = (x0[:, 0] + 1j * x0[:, 1]) * np.exp(1j * om * T)
+        errs.append(np.abs(x[:, 0] + 1j * x[:, 1] - exact).max())
+    rates = [np.log2(errs[i] / errs[i + 1]) for i in range(2)]
+    assert all(3.8 < r < 4.3 for r in rates), (errs, rates)
