@@ -217,6 +217,14 @@ int alegb_set_max_ctas(alegb_ctx* ctx, int max_ctas);
  * dynamic shared memory in bytes}.  ALEGB_UNSUPPORTED if there is no such kernel.  Needs no context and no device
  * (tests/test_pipe_protocol.py simulates the protocol with these numbers). */
 int alegb_pipe_config(int dim, int N, int* cfg);
+/* Absorbing layer (a8): where the pipelined stage kernel runs and has an instantiation for it, the auxiliary fields of
+ * the layer elements are advanced INSIDE the stage kernel (their D_a q, exterior traces and metrics are already on
+ * chip there): the quads outside the layer run through the plain instantiation, the quads that touch the layer
+ * through a second launch that also advances their auxiliary fields.  on = 0 selects the separate layer kernel after
+ * the stage kernel.  Default: on in 3-D, off in 2-D (where the layer is a thin ring and the split costs more than the
+ * fusion saves; measured in profiles/r2_layer_fusion.md).  Same equations (reading R12); results agree to round-off (summation order of the LIFT
+ * contraction is the same, the volume part is formed per direction in both). */
+int alegb_set_layer_fusion(alegb_ctx* ctx, int on);
 /* Inside a step the vertex-motion and geometric-factor kernels (a1, a2) of stage i+1 depend on time only; with the
  * overlap on (default) they run on a stream of the library's own beside the stage kernel of stage i, into a second
  * set of geometry arrays, joined by events (captured into the step graph as a parallel branch).  Same kernels, same

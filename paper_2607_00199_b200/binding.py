@@ -36,6 +36,7 @@ _SIGNATURES = {
     "alegb_set_coordinate_mode": (_c.c_int, [_P, _c.c_int, _c.c_double]),
     "alegb_set_relaxation": (_c.c_int, [_P, _c.c_int]),
     "alegb_set_geometry_overlap": (_c.c_int, [_P, _c.c_int]),
+    "alegb_set_layer_fusion": (_c.c_int, [_P, _c.c_int]),
     "alegb_wall_forces": (_c.c_int, [_P, _c.c_double, _P, _c.c_int, _P, _P, _P]),
     "alegb_get_cubature": (_c.c_int, [_P, _c.POINTER(_c.c_int), _c.POINTER(_c.c_int), _P, _P, _P, _P]),
     "alegb_get_positions": (_c.c_int, [_P, _P, _P]),
@@ -165,6 +166,9 @@ class Context:
 
     def alegb_set_geometry_overlap(self, on):
         self._check(_lib.alegb_set_geometry_overlap(self._h, int(bool(on))))
+
+    def alegb_set_layer_fusion(self, on):
+        self._check(_lib.alegb_set_layer_fusion(self._h, int(bool(on))))
 
     def alegb_set_relaxation(self, mode):
         self._check(_lib.alegb_set_relaxation(self._h, int(mode)))

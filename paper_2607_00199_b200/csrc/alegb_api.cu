@@ -30,6 +30,10 @@ struct alegb_ctx {
   bool cub_mma_ok = false;  // a DMMA cubature kernel exists for (dim, N)
   bool pipe_ok = false;  // a pipelined DMMA stage kernel exists for (dim, N)
   bool pml_mma_ok = false;  // a DMMA kernel for the absorbing layer's auxiliary fields exists for (dim, N)
+  bool pipe_layer_ok = false;  // the pipelined stage kernel has an instantiation with the absorbing layer fused in
+  bool fuse_layer = true;      // alegb_set_layer_fusion
+  // a8 inside the stage kernel (one launch per stage instead of two) where the pipelined kernel runs and supports it
+  bool layer_fused() const { return Kpml > 0 && fuse_layer && pipe_ok && pipe_layer_ok && kernel_mode != 1; }
   int kernel_mode = 0;   // 0 auto (pipelined DMMA, else generic), 1 generic, 2 pipelined DMMA
   // device: mesh
   double *d_X0 = nullptr, *d_xv = nullptr, *d_vv = nullptr;
@@ -57,6 +61,8 @@ struct alegb_ctx {
   double* sg() const { return geo_buf ? d_sgeo1 : d_sgeo; }
   double* vvl() const { return geo_buf ? d_vvel1 : d_vvel; }
   int32_t *d_pml_index = nullptr, *d_pml_elems = nullptr;
+  int32_t *d_quads_layer = nullptr, *d_quads_plain = nullptr;   // quads that touch the absorbing layer / the others
+  int64_t nquads_layer = 0, nquads_plain = 0;
   double* d_pml_sigma = nullptr;
   // device: step workspace
   double *d_Q1 = nullptr, *d_Q2 = nullptr, *d_F0 = nullptr, *d_ACC = nullptr, *d_Qhost = nullptr;
@@ -119,6 +125,7 @@ void free_mesh(alegb_ctx* ctx) {
   dev_free(ctx->d_EToB); dev_free(ctx->d_vgeo); dev_free(ctx->d_sgeo); dev_free(ctx->d_vvel);
   dev_free(ctx->d_vgeo1); dev_free(ctx->d_sgeo1); dev_free(ctx->d_vvel1); ctx->geo_buf = 0;
   dev_free(ctx->d_pml_index); dev_free(ctx->d_pml_elems); dev_free(ctx->d_pml_sigma);
+  dev_free(ctx->d_quads_layer); dev_free(ctx->d_quads_plain); ctx->nquads_layer = ctx->nquads_plain = 0;
   dev_free(ctx->d_Q1); dev_free(ctx->d_Q2); dev_free(ctx->d_F0); dev_free(ctx->d_ACC); dev_free(ctx->d_Qhost);
   dev_free(ctx->d_AUX); dev_free(ctx->d_AUXS); dev_free(ctx->d_AUXACC);
   ctx->mesh_ready = false;
@@ -182,6 +189,12 @@ void fill_common(const alegb_ctx* ctx, PmlArgs& a) {
   a.c = ctx->c;
   for (int k = 0; k < kMaxFields; ++k) a.q_inf[k] = ctx->q_inf[k];
 }
+// the auxiliary-field part of a stage handed to the stage kernel (LAYER instantiation of stage_pipe.cu)
+void layer_from(const PmlArgs& p, LayerArgs& l) {
+  l.on = true;
+  l.aux_n = p.aux_n; l.acc_in = p.acc_in; l.G_out = p.G_out; l.aux_out = p.aux_out; l.acc_out = p.acc_out;
+  l.cx_n = p.cx_n; l.cx_acc = p.cx_acc; l.cx_g = p.cx_g; l.cy_n = p.cy_n; l.cy_acc = p.cy_acc; l.cy_g = p.cy_g;
+}
 // a8: the DMMA kernel unless the generic kernels were asked for (alegb_set_kernel(1)) or (dim, N) has none
 cudaError_t launch_pml_any(const alegb_ctx* ctx, const PmlArgs& p, cudaStream_t s) {
   if (ctx->pml_mma_ok && ctx->kernel_mode != 1) return launch_pml_mma(ctx->ref.dim, ctx->ref.N, p, ctx->ctas(), s);
@@ -225,7 +238,18 @@ int timed_stage(alegb_ctx* ctx, const StageArgs& a_in, cudaStream_t s) {
     a.relax_cub = ctx->d_R;
   }
   const int mode = ctx->kernel_mode;
-  if (ctx->pipe_ok && (mode == 0 || mode == 2)) CU(launch_stage_pipe(ctx->ref.dim, ctx->ref.N, a, ctx->ctas(), s));
+  if (ctx->pipe_ok && (mode == 0 || mode == 2)) {
+    if (a.layer.on) {
+      // the quads outside the layer through the plain instantiation (deep ring, small slots), then the quads that
+      // touch it through the LAYER instantiation (a8 fused in)
+      StageArgs b = a;
+      b.layer.on = false; b.quad_list = ctx->d_quads_plain; b.nquads_list = ctx->nquads_plain;
+      CU(launch_stage_pipe(ctx->ref.dim, ctx->ref.N, b, ctx->ctas(), s));
+      ctx->launches++;
+      a.quad_list = ctx->d_quads_layer; a.nquads_list = ctx->nquads_layer;
+    }
+    CU(launch_stage_pipe(ctx->ref.dim, ctx->ref.N, a, ctx->ctas(), s));
+  }
   else CU(launch_stage(ctx->ref.dim, ctx->ref.N, a, ctx->ctas(), s));
   ctx->launches++;
   if (rec) {
@@ -323,11 +347,9 @@ int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t
       cf.cq_acc = 1.0;
       for (int k = 0; k < Nf; ++k) cf.cq_f[k] = dt * B(k, 3);
     }
-    rc = timed_stage(ctx, a, s);
-    if (rc != ALEGB_OK) return rc;
+    PmlArgs p;
     if (pml) {
       // auxiliary fields: Lambda = 0, classic RK4 weights (reading R12)
-      PmlArgs p;
       fill_common(ctx, p);
       p.q_in = a.q_in;
       p.aux_in = i == 0 ? ctx->d_AUX : ctx->d_AUXS;
@@ -339,6 +361,11 @@ int sark_step(alegb_ctx* ctx, const double* q_n, double* const outs[4], double t
       } else {
         p.acc_in = ctx->d_AUXACC; p.aux_out = ctx->d_AUX; p.cx_acc = 1.0; p.cx_g = dt * (1.0 / 6.0);
       }
+      if (ctx->layer_fused()) layer_from(p, a.layer);   // a8 inside the stage kernel
+    }
+    rc = timed_stage(ctx, a, s);
+    if (rc != ALEGB_OK) return rc;
+    if (pml && !a.layer.on) {
       CU(launch_pml_any(ctx, p, s));
       ctx->launches++;
     }
@@ -434,6 +461,10 @@ int alegb_create(alegb_ctx** out, int dim, int N, int cuda_device) {
   struct { int NB, KS; } L{(Np + 7) / 8, (Np + 3) / 4};   // node blocks of 8 rows, k-steps of 4 columns
   ctx->pipe_ok = configure_stage_pipe(dim, N) == cudaSuccess;
   ctx->pml_mma_ok = configure_pml_mma(dim, N) == cudaSuccess;
+  ctx->pipe_layer_ok = ctx->pipe_ok && stage_pipe_layer_supported(dim, N);
+  // measured (profiles/r2_layer_fusion.md): config 5 (3-D N=3) 32.4 -> 34.3 GDOF-stage/s fused, config 3 (2-D N=4)
+  // 69.5 -> 63.5: the 2-D layer is a thin ring and a second small launch costs more than the fusion saves
+  ctx->fuse_layer = dim == 3;
   cudaGetLastError();
   if (ctx->pipe_ok || ctx->pml_mma_ok) {
     std::vector<double> Av((size_t)dim * L.NB * L.KS * 32, 0.0);
@@ -573,6 +604,17 @@ int alegb_mesh_upload(alegb_ctx* ctx, int64_t Nverts, const double* X0, int64_t 
     CU(upload(ctx, &ctx->d_pml_index, pml_index.data(), pml_index.size()));
     CU(upload(ctx, &ctx->d_pml_elems, ctx->pml_elems_host.data(), ctx->pml_elems_host.size()));
     CU(upload(ctx, &ctx->d_pml_sigma, sig.data(), sig.size()));
+    {   // quads of 4 consecutive elements, split by whether any of them lies in the layer
+      std::vector<int32_t> ql, qp;
+      for (int64_t qd = 0; qd < (K + 3) / 4; ++qd) {
+        bool in = false;
+        for (int64_t e = 4 * qd; e < K && e < 4 * qd + 4; ++e) in |= pml_index[e] >= 0;
+        (in ? ql : qp).push_back((int32_t)qd);
+      }
+      ctx->nquads_layer = (int64_t)ql.size(); ctx->nquads_plain = (int64_t)qp.size();
+      CU(upload(ctx, &ctx->d_quads_layer, ql.data(), ql.size()));
+      CU(upload(ctx, &ctx->d_quads_plain, qp.data(), qp.size()));
+    }
     CU(dev_alloc(ctx, &ctx->d_AUX, na));
     CU(dev_alloc(ctx, &ctx->d_AUXS, na));
     CU(dev_alloc(ctx, &ctx->d_AUXACC, na));
@@ -793,12 +835,15 @@ int alegb_rhs_pml(alegb_ctx* ctx, double t, const double* d_q, const double* d_a
   fill_common(ctx, a);
   a.q_in = d_q; a.F_out = d_F;
   a.aux = ctx->Kpml > 0 ? (d_aux ? d_aux : ctx->d_AUX) : nullptr;
-  rc = timed_stage(ctx, a, s);
-  if (rc != ALEGB_OK) return rc;
+  PmlArgs p;
   if (d_Faux && ctx->Kpml > 0) {
-    PmlArgs p;
     fill_common(ctx, p);
     p.q_in = d_q; p.aux_in = a.aux; p.G_out = d_Faux;
+    if (ctx->layer_fused()) layer_from(p, a.layer);
+  }
+  rc = timed_stage(ctx, a, s);
+  if (rc != ALEGB_OK) return rc;
+  if (d_Faux && ctx->Kpml > 0 && !a.layer.on) {
     CU(launch_pml_any(ctx, p, s));
     ctx->launches++;
   }
@@ -979,6 +1024,13 @@ int alegb_pipe_config(int dim, int N, int* cfg) {
   if (!stage_pipe_config(dim, N, c)) return ALEGB_UNSUPPORTED;
   cfg[0] = c.producer_groups; cfg[1] = c.slots; cfg[2] = c.items_per_quad; cfg[3] = c.consumer_warps;
   cfg[4] = c.warps_per_group; cfg[5] = c.producer_warps; cfg[6] = c.elements_per_quad; cfg[7] = c.smem_bytes;
+  return ALEGB_OK;
+}
+
+int alegb_set_layer_fusion(alegb_ctx* ctx, int on) {
+  if (!ctx) return ALEGB_INVALID_ARG;
+  ctx->fuse_layer = on != 0;
+  ctx->config_version++;
   return ALEGB_OK;
 }
 

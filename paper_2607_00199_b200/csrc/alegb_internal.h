@@ -25,6 +25,16 @@ struct StageCoef {
   double cq_acc, ca_acc;
 };
 
+// a8 fused into the pipelined stage kernel (stage_pipe.cu, LAYER instantiation): the auxiliary fields of the absorbing
+// layer [Kpml][dim][Nf][Np] (reading R12).  G = right-hand side of the auxiliary equation evaluated on StageArgs::aux;
+//   aux_out = cx_n aux_n + cx_acc acc_in + cx_g G ;  acc_out = cy_n aux_n + cy_acc acc_in + cy_g G
+struct LayerArgs {
+  bool on;                 // run the fused path (false: the stage kernel only subtracts sigma_d q~^d from F)
+  const double* aux_n; const double* acc_in;
+  double* G_out; double* aux_out; double* acc_out;
+  double cx_n, cx_acc, cx_g, cy_n, cy_acc, cy_g;
+};
+
 struct StageArgs {
   // mesh / geometry at the stage time
   int64_t K;
@@ -56,6 +66,9 @@ struct StageArgs {
   double* q_out;
   double* acc_out;
   StageCoef coef;
+  LayerArgs layer;
+  const int32_t* quad_list;   // pipelined kernel: the quads (groups of 4 consecutive elements) of this launch, or NULL = all
+  int64_t nquads_list;
 };
 
 // cubature-projected relaxation (cubature.cu): R[K][Ns][Np] = P N~(I q), Ns = dim (dim+1)/2 stiff fields
@@ -134,5 +147,6 @@ cudaError_t configure_stage_pipe(int dim, int N);     // cudaErrorInvalidValue i
 cudaError_t launch_stage_pipe(int dim, int N, const StageArgs& a, int num_sms, cudaStream_t s);
 struct PipeConfig { int producer_groups, slots, items_per_quad, consumer_warps, warps_per_group, producer_warps, elements_per_quad, smem_bytes; };
 bool stage_pipe_config(int dim, int N, PipeConfig& c);   // false if (dim, N) has no such kernel
+bool stage_pipe_layer_supported(int dim, int N);          // the instantiation with the absorbing layer fused in exists
 
 }  // namespace alegb

@@ -31,7 +31,9 @@ __host__ __device__ constexpr int stride_pad(int x) {
   return s;
 }
 
-template <int DIM, int N>
+// LAYER: the instantiation for meshes with an absorbing layer (a8 fused in, see the consumers): a slot carries DIM
+// more flux tiles (the directional pieces of reading R12), so the ring is as deep as shared memory allows.
+template <int DIM, int N, bool LAYER = false>
 struct Cfg {
   static constexpr int Np = DIM == 2 ? (N + 1) * (N + 2) / 2 : (N + 1) * (N + 2) * (N + 3) / 6;
   static constexpr int Nfp = DIM == 2 ? N + 1 : (N + 1) * (N + 2) / 2;
@@ -54,9 +56,10 @@ struct Cfg {
   // barrier -> flux) is what bounds the kernel (profiles/r1_v12_cfg3_stage_kernel.md), so every producer warp
   // streams quads of its own (warp w takes quads w, w+6, ...) into a 16-slot ring.  3-D N <= 3 sits in between:
   // two groups of two warps, ring of 8 (config 5: stage kernel 4.94 -> 4.56 ms).
-  static constexpr int PG = DIM == 2 ? 32 : (N <= 3 ? 64 : PW * 32);   // threads of one producer group
-  static constexpr int NS = PG == 32 ? 16 : (PG == 64 ? 8 : 4);   // slots in the ring
+  static constexpr int PG = DIM == 2 ? 32 : (N <= 3 && !LAYER ? 64 : PW * 32);   // threads of one producer group
+  static constexpr int NS_want = PG == 32 ? 16 : (PG == 64 ? 8 : 4);   // slots in the ring, if they fit
   static constexpr int NG = PW * 32 / PG;      // producer groups
+  static constexpr int NTILE = LAYER ? 1 + DIM : 1;   // flux tiles per slot: the full flux (+ one per direction)
   static constexpr int TAG0 = PG >= 64 ? 32 : EG;   // first thread of a group that fetches boundary tags
   static constexpr int Threads = (PW + CW) * 32;
   static constexpr int PT = PG;                // threads producing one quad
@@ -68,7 +71,8 @@ struct Cfg {
   static constexpr int SGE = Nfaces * (DIM + 2);   // sgeo: per face unit normal, sJ, Fscale
   // slot layout, in doubles
   static constexpr int off_gt = EG * Nf * S;
-  static constexpr int off_vg = off_gt + EG * Nf * SG;
+  static constexpr int tile_doubles = EG * Nf * SG;
+  static constexpr int off_vg = off_gt + NTILE * tile_doubles;
   static constexpr int off_vv = off_vg + EG * VG;
   static constexpr int off_sg = off_vv + EG * VV;
   static constexpr int off_int = off_sg + EG * SGE;          // ints: pml[EG], tag[EG*Nfaces]
@@ -76,9 +80,11 @@ struct Cfg {
   static constexpr int avol_doubles = DIM * NB * KS * 32;
   static constexpr int alift_doubles = NB * KFT * 32;
   static constexpr int lam_doubles = NB * 8 * (DIM + 1);
-  static constexpr size_t smem_bytes = (size_t)(avol_doubles + alift_doubles + lam_doubles + NS * slot_doubles) * 8 +
-                                       (size_t)NFN * 4 + 2 * NS * 8 + 16;
-  static constexpr bool supported = smem_bytes <= 227 * 1024;
+  static constexpr size_t fixed_bytes = (size_t)(avol_doubles + alift_doubles + lam_doubles) * 8 + (size_t)NFN * 4 + 16;
+  static constexpr int NS_fit = (int)((227 * 1024 - fixed_bytes) / ((size_t)slot_doubles * 8 + 16));
+  static constexpr int NS = NS_want < NS_fit ? NS_want : NS_fit;
+  static constexpr size_t smem_bytes = fixed_bytes + (size_t)NS * slot_doubles * 8 + 2 * (NS > 0 ? NS : 0) * 8;
+  static constexpr bool supported = NS >= NG && NS >= (LAYER ? 3 : 2);
 };
 
 __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b) {
@@ -123,10 +129,10 @@ __device__ __forceinline__ void producer_sync(int group) {   // the threads of o
 
 }  // namespace pipe
 
-template <int DIM, int N>
-__global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kernel(StageArgs a) {
+template <int DIM, int N, bool LAYER>
+__global__ void __launch_bounds__(pipe::Cfg<DIM, N, LAYER>::Threads, 1) stage_pipe_kernel(StageArgs a) {
   using namespace pipe;
-  using C = Cfg<DIM, N>;
+  using C = Cfg<DIM, N, LAYER>;
   constexpr int Np = C::Np, Nfp = C::Nfp, Nfaces = C::Nfaces, NFN = C::NFN, Nf = C::Nf, NT = C::NT, NB = C::NB;
   constexpr int KS = C::KS, KFT = C::KFT, S = C::S, SG = C::SG, EG = C::EG, NS = C::NS, PT = C::PT;
   extern __shared__ double smem[];
@@ -159,7 +165,14 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
   __syncthreads();
 
   const double cs = a.c;
-  const int64_t nquads = (a.K + EG - 1) / EG;
+  // the quads of this launch: all of the mesh, or a list (meshes with an absorbing layer run the plain instantiation
+  // over the quads outside the layer and the LAYER instantiation over the quads that touch it)
+  const int64_t nquads = a.quad_list != nullptr ? a.nquads_list : (a.K + EG - 1) / EG;
+  auto quad_of = [&](int ql) -> int64_t {
+    const int64_t idx = (int64_t)ql * gridDim.x + blockIdx.x;
+    if (a.quad_list == nullptr) return idx;
+    return idx < nquads ? (int64_t)__ldg(a.quad_list + idx) : 0;
+  };
   const int nq_cta = (int)((nquads - blockIdx.x + gridDim.x - 1) / gridDim.x);   // quads blockIdx.x + ql*gridDim.x
 
   if (warp < C::PW) {
@@ -180,7 +193,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
     int meta_next = 0;      // pml index (threads < EG) / boundary tag (threads TAG0 .. TAG0+EG*Nfaces) of that quad
 
     auto load_indices = [&](int ql) {
-      const int64_t e0 = ((int64_t)ql * gridDim.x + blockIdx.x) * EG;
+      const int64_t e0 = quad_of(ql) * EG;
 #pragma unroll
       for (int r = 0; r < ROUNDS; ++r) {
         const int64_t ee = e0 + task_fe[r];
@@ -188,7 +201,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       }
     };
     auto issue = [&](int ql) {
-      const int64_t e0 = ((int64_t)ql * gridDim.x + blockIdx.x) * EG;
+      const int64_t e0 = quad_of(ql) * EG;
       const int nel = (a.K - e0) < EG ? (int)(a.K - e0) : EG;
       const int slot = ql % NS, use = ql / NS;
       double* qt = sslots + slot * C::slot_doubles;
@@ -241,7 +254,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
     if (grp < nq_cta) issue(grp);
     cp_async_commit();
     for (int ql = grp; ql < nq_cta; ql += C::NG) {
-      const int64_t e0 = ((int64_t)ql * gridDim.x + blockIdx.x) * EG;
+      const int64_t e0 = quad_of(ql) * EG;
       const int nel = (a.K - e0) < EG ? (int)(a.K - e0) : EG;
       const int slot = ql % NS;
       double* qt = sslots + slot * C::slot_doubles;
@@ -292,6 +305,29 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
         upwind_flux<DIM>(qM, qP, nh, cs, vn, Fscale, fl);
 #pragma unroll
         for (int k = 0; k < Nf; ++k) gt[(fe * Nf + k) * SG + m] = fl[k];
+        if constexpr (LAYER) {
+          // a8 (reading R12): the directional pieces Fscale ( -1/2 n_d c A^_d [q] + 1/2 n_d^2 |A_n| [q] ) of the quads
+          // that touch the absorbing layer, one more flux tile per direction
+          bool inlayer = false;
+#pragma unroll
+          for (int el = 0; el < EG; ++el) inlayer |= si[el] >= 0;
+          if (inlayer) {
+            if (r == 0 && pt < EG && si[pt] >= 0) {   // pull the element's auxiliary rows towards L2 for the consumers
+              const int64_t off = (int64_t)si[pt] * DIM * Nf * Np;
+              const uint32_t bytes = (uint32_t)(DIM * Nf * Np * 8);
+              prefetch_l2(a.aux + off, bytes);
+              if (a.layer.aux_n != nullptr && a.layer.aux_n != a.aux) prefetch_l2(a.layer.aux_n + off, bytes);
+              if (a.layer.acc_in != nullptr) prefetch_l2(a.layer.acc_in + off, bytes);
+            }
+#pragma unroll
+            for (int dd = 0; dd < DIM; ++dd) {
+              double fd2[Nf];
+              directional_flux<DIM>(dd, qM, qP, nh, cs, Fscale, fd2);
+#pragma unroll
+              for (int k = 0; k < Nf; ++k) gt[(1 + dd) * C::tile_doubles + (fe * Nf + k) * SG + m] = fd2[k];
+            }
+          }
+        }
       }
       mbar_arrive(&full[slot]);
     }
@@ -322,7 +358,7 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
       const int ql = it / NB, nb = it - ql * NB;
       pass_quads(ql);
       next_q = ql + 1;
-      const int64_t quad = (int64_t)ql * gridDim.x + blockIdx.x;
+      const int64_t quad = quad_of(ql);
       const int64_t e0 = quad * EG;
       const int nel = (a.K - e0) < EG ? (int)(a.K - e0) : EG;
       const int slot = ql % NS, use = ql / NS;
@@ -435,8 +471,15 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
 #pragma unroll
         for (int t = 0; t < NT; ++t) dmma(V[t][0], V[t][1], af, bf[t]);
       }
-      // all reads of the slot are done
-      mbar_arrive(&empty[slot]);
+      // all reads of the slot are done (quads in the absorbing layer: after their directional contractions below)
+      bool inlayer = false;
+      if constexpr (LAYER) {
+        if (a.layer.on) {
+#pragma unroll
+          for (int el = 0; el < EG; ++el) inlayer |= si[el] >= 0;
+        }
+      }
+      if (!inlayer) mbar_arrive(&empty[slot]);
       // ---- a6: SARK stage update (L132-134), straight from the accumulator registers; one uniform branch per output
       if (evalid) {
         if (a.F_out != nullptr) {
@@ -469,26 +512,122 @@ __global__ void __launch_bounds__(pipe::Cfg<DIM, N>::Threads, 1) stage_pipe_kern
         if (a.q_out != nullptr) combine(a.coef.cq_n, a.coef.cq_f0, a.coef.cq_acc, a.coef.cq_f, a.q_out + base);
         if (a.acc_out != nullptr) combine(a.coef.ca_n, a.coef.ca_f0, a.coef.ca_acc, a.coef.ca_f, a.acc_out + base);
       }
+      if constexpr (LAYER) {
+        if (inlayer) {
+          // ---- a8, fused: auxiliary fields of the absorbing layer (reading R12) for the layer elements of this quad,
+          //   d/dt q~^d = -c A^_d d_d q + LIFT( directional flux tile d ) - sigma_d q~^d,   classic RK4 weights.
+          // D_a q is still in the accumulator registers and the exterior traces were gathered once for all tiles;
+          // the separate kernel (pml_mma.cu) re-read the q tile, re-gathered q+ and repeated the D_a contraction.
+          const int64_t p = pml >= 0 ? pml : 0;          // clamped: valid addresses in every lane, stores predicated
+          const bool pvalid = evalid && pml >= 0;
+          double Vd[DIM][NT][2];
+          {   // volume parts -c A^_dd d_dd q of all directions on the accumulator registers (D_a q is dead afterwards)
+            double Gm[DIM * DIM];
+#pragma unroll
+            for (int x = 0; x < DIM * DIM; ++x) Gm[x] = svg[x];
+#pragma unroll
+            for (int dd = 0; dd < DIM; ++dd) {
+              double st[Nf];
+              hermite_apply<DIM>(
+                  [&](int d, int j) {
+                    if (d != dd) return 0.0;
+                    double s = 0.0;
+#pragma unroll
+                    for (int r = 0; r < DIM; ++r) s = fma(Gm[r * DIM + dd], acc[r][j >> 1][j & 1], s);
+                    return s;   // d q_j / d x_dd
+                  },
+                  st);
+#pragma unroll
+              for (int k = 0; k < Nf; ++k) Vd[dd][k >> 1][k & 1] = -cs * st[k];
+            }
+          }
+          // surface parts: LIFT of the directional flux tiles, all directions back to back, then the slot is free
+#pragma unroll
+          for (int dd = 0; dd < DIM; ++dd) {
+            const double* gd = gt + (1 + dd) * C::tile_doubles;
+#pragma unroll
+            for (int ks = 0; ks < KFT; ++ks) {
+              double bf[NT];
+#pragma unroll
+              for (int t = 0; t < NT; ++t) bf[t] = gd[(bcol + 2 * t) * SG + 4 * ks + c];
+              const double af = sAlift[(nb * KFT + ks) * 32 + lane];
+#pragma unroll
+              for (int t = 0; t < NT; ++t) dmma(Vd[dd][t][0], Vd[dd][t][1], af, bf[t]);
+            }
+          }
+          mbar_arrive(&empty[slot]);
+          // RK combination of the auxiliary state, direction by direction (straight-line loads behind uniform branches)
+#pragma unroll
+          for (int dd = 0; dd < DIM; ++dd) {
+            const double sig = a.pml_sigma[p * DIM + dd];
+            const int64_t pb = ((p * DIM + dd) * Nf) * Np + nn;
+            double xi[Nf], xn[Nf], xa[Nf];
+            {
+              const double* pi = a.aux + pb;
+#pragma unroll
+              for (int k = 0; k < Nf; ++k) xi[k] = pi[k * Np];
+            }
+#pragma unroll
+            for (int k = 0; k < Nf; ++k) { xn[k] = 0.0; xa[k] = 0.0; }
+            if (a.layer.aux_n != nullptr) {
+              if (a.layer.aux_n == a.aux) {
+#pragma unroll
+                for (int k = 0; k < Nf; ++k) xn[k] = xi[k];
+              } else {
+                const double* pn = a.layer.aux_n + pb;
+#pragma unroll
+                for (int k = 0; k < Nf; ++k) xn[k] = pn[k * Np];
+              }
+            }
+            if (a.layer.acc_in != nullptr) {
+              const double* pa = a.layer.acc_in + pb;
+#pragma unroll
+              for (int k = 0; k < Nf; ++k) xa[k] = pa[k * Np];
+            }
+            if (pvalid) {
+#pragma unroll
+              for (int k = 0; k < Nf; ++k) {
+                const int64_t idx = pb + k * Np;
+                const double gg = Vd[dd][k >> 1][k & 1] - sig * xi[k];
+                if (a.layer.G_out) a.layer.G_out[idx] = gg;
+                if (a.layer.aux_out) a.layer.aux_out[idx] = fma(a.layer.cx_g, gg, fma(a.layer.cx_acc, xa[k], a.layer.cx_n * xn[k]));
+                if (a.layer.acc_out) a.layer.acc_out[idx] = fma(a.layer.cy_g, gg, fma(a.layer.cy_acc, xa[k], a.layer.cy_n * xn[k]));
+              }
+            }
+          }
+        }
+      }
     }
     pass_quads(nq_cta);
   }
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-template <int DIM, int N>
-static cudaError_t launch_pipe_one(const StageArgs& a, int num_sms, cudaStream_t s, bool configure_only) {
-  using C = pipe::Cfg<DIM, N>;
+template <int DIM, int N, bool LAYER>
+static cudaError_t launch_pipe_inst(const StageArgs& a, int num_sms, cudaStream_t s, bool configure_only) {
+  using C = pipe::Cfg<DIM, N, LAYER>;
   if constexpr (!C::supported) {
     return cudaErrorInvalidValue;
   } else {
     if (configure_only)
-      return cudaFuncSetAttribute(stage_pipe_kernel<DIM, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
-    const int64_t nquads = (a.K + C::EG - 1) / C::EG;
+      return cudaFuncSetAttribute(stage_pipe_kernel<DIM, N, LAYER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
+    const int64_t nquads = a.quad_list != nullptr ? a.nquads_list : (a.K + C::EG - 1) / C::EG;
     if (nquads == 0) return cudaSuccess;
     int64_t grid = nquads < num_sms ? nquads : num_sms;
-    stage_pipe_kernel<DIM, N><<<(int)grid, C::Threads, C::smem_bytes, s>>>(a);
+    stage_pipe_kernel<DIM, N, LAYER><<<(int)grid, C::Threads, C::smem_bytes, s>>>(a);
     return cudaGetLastError();
   }
+}
+// a.layer.on selects the instantiation with the absorbing layer fused in (configure: both, the plain one decides)
+template <int DIM, int N>
+static cudaError_t launch_pipe_one(const StageArgs& a, int num_sms, cudaStream_t s, bool configure_only) {
+  if (configure_only) {
+    cudaError_t e = launch_pipe_inst<DIM, N, false>(a, num_sms, s, true);
+    if (e == cudaSuccess && pipe::Cfg<DIM, N, true>::supported) e = launch_pipe_inst<DIM, N, true>(a, num_sms, s, true);
+    return e;
+  }
+  if (a.layer.on) return launch_pipe_inst<DIM, N, true>(a, num_sms, s, false);
+  return launch_pipe_inst<DIM, N, false>(a, num_sms, s, false);
 }
 
 #define ALEGB_PIPE_DISPATCH(...)                                  \
@@ -512,12 +651,26 @@ cudaError_t configure_stage_pipe(int dim, int N) {
   StageArgs a{};
   ALEGB_PIPE_DISPATCH(a, 0, nullptr, true)
 }
+bool stage_pipe_layer_supported(int dim, int N) {
+  switch (dim * 10 + N) {
+    case 21: return pipe::Cfg<2, 1, true>::supported;
+    case 22: return pipe::Cfg<2, 2, true>::supported;
+    case 23: return pipe::Cfg<2, 3, true>::supported;
+    case 24: return pipe::Cfg<2, 4, true>::supported;
+    case 25: return pipe::Cfg<2, 5, true>::supported;
+    case 31: return pipe::Cfg<3, 1, true>::supported;
+    case 32: return pipe::Cfg<3, 2, true>::supported;
+    case 33: return pipe::Cfg<3, 3, true>::supported;
+    case 34: return pipe::Cfg<3, 4, true>::supported;
+    default: return false;
+  }
+}
 
 // The hand-over parameters of Cfg<DIM,N>, for tests/test_pipe_protocol.py (alegb_pipe_config): the simulation must
 // model the kernel that is compiled, not a re-typed copy of its constants.
 template <int DIM, int N>
 static bool pipe_config_one(PipeConfig& c) {
-  using C = pipe::Cfg<DIM, N>;
+  using C = pipe::Cfg<DIM, N, false>;
   if (!C::supported) return false;
   c.producer_groups = C::NG; c.slots = C::NS; c.items_per_quad = C::NB; c.consumer_warps = C::CW;
   c.warps_per_group = C::PG / 32; c.producer_warps = C::PW; c.elements_per_quad = C::EG; c.smem_bytes = (int)C::smem_bytes;

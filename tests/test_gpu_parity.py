@@ -743,3 +743,37 @@ def test_user_stage_velocities_that_depend_on_the_positions_match_oracle(refs, B
         assert rel_linf(dq.cpu().numpy(), qo) <= 2 * TOL_STAGE   # second step: each side continues from its own state
         assert np.abs(dx.cpu().numpy() - x).max() <= 1e-14 * np.abs(x).max()
     ctx.close()
+
+
+# ------------------------------------------------------------------ a8 fused into the stage kernel
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", ["cfg3", "cfg5", "cfg5_tiny"])
+def test_layer_fusion_agrees_with_the_separate_layer_kernel(name, refs, B):
+    """alegb_set_layer_fusion: the auxiliary fields advanced inside the pipelined stage kernel (default) against the
+    separate layer kernel after it -- same equations (reading R12), F and G to round-off, ten steps of q and of the
+    auxiliary state.  (Both paths are compared with the oracle by the other tests: the default is the fused one.)"""
+    ref, cfg = make_case(name, refs)
+    q = perturbed(cfg)
+    rng = np.random.default_rng(11)
+    out = {}
+    for fused in (1, 0):
+        ctx = B.context_from_config(cfg)
+        ctx.alegb_set_layer_fusion(fused)
+        Kpml = ctx.alegb_pml_count()
+        assert Kpml > 0
+        aux = 1e-3 * np.random.default_rng(11).standard_normal((Kpml, cfg["dim"]) + q.shape[1:])
+        dq, dF = dev(q), torch.empty(q.shape, dtype=torch.float64, device="cuda")
+        dG = torch.empty(aux.shape, dtype=torch.float64, device="cuda")
+        n0 = ctx.alegb_launch_count()
+        ctx.alegb_rhs_pml(0.3, dq, dev(aux), dF, dG)
+        nl = ctx.alegb_launch_count() - n0
+        ctx.alegb_pml_set(dev(aux))
+        ctx.alegb_step(dq, 0.0, cfg["dt"], 10)
+        da = torch.empty_like(dG)
+        ctx.alegb_pml_get(da)
+        torch.cuda.synchronize()
+        out[fused] = (dF, dG, dq, da, nl)
+        ctx.close()
+    assert out[1][4] <= out[0][4]                              # the layer quads run through one (fused) launch
+    for x, y in zip(out[1][:4], out[0][:4]):
+        assert (x - y).abs().max().item() <= 1e-13 * max(y.abs().max().item(), 1e-300)
