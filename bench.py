@@ -49,7 +49,13 @@ ALGO_BYTES_PER_DOF_STAGE = 38.0          # 152 B per DOF-step
 POINTWISE_FLOP_PER_DOF_STAGE = 50.0
 # dram__bytes_read.sum + dram__bytes_write.sum of the stage kernel per launch from committed `ncu --set full` captures
 # (mean over the stages of a step); configurations without a capture report no traffic figure.
-NCU_DRAM_BYTES_PER_LAUNCH = {4: (2.505e9, "profiles/r1_v8_pipe_stage_kernel.md")}
+NCU_DRAM_BYTES_PER_LAUNCH = {
+    4: (2.507e9, "profiles/r2_final.md"),
+    # config 5: both stage launches of a stage (quads outside + inside the absorbing layer); includes a8's auxiliary
+    # arrays (up to 5 arrays x 3 directions x 8 B per layer DOF), which the 38 B per DOF-stage do not count
+    5: (21.94e9, "profiles/r2_final.md"),
+    3: (161.3e6, "profiles/r2_final.md"),
+    2: (17.5e6, "profiles/r2_final.md")}
 DIM_N = {1: (2, 3), 2: (2, 4), 3: (2, 4), 4: (3, 4), 5: (3, 3)}
 
 
