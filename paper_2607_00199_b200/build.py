@@ -52,13 +52,21 @@ def build(force=False, verbose=False):
         if force or _newer(o, [s] + headers):
             _run([CXX] + CXX_FLAGS + ["-c", s, "-o", o], verbose, log)
         objs.append(o)
+    jobs = []
     for src in CU_SOURCES:
         s, o = os.path.join(CSRC, src), os.path.join(OBJ, src + ".o")
         if not os.path.exists(s):
             continue
         if force or _newer(o, [s] + headers):
-            _run([NVCC] + NVCC_FLAGS + ["-c", s, "-o", o], verbose, log)
+            jobs.append([NVCC] + NVCC_FLAGS + ["-c", s, "-o", o])
         objs.append(o)
+    if jobs:   # the translation units are independent: compile them side by side
+        from concurrent.futures import ThreadPoolExecutor
+        with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 1)) as pool:
+            logs = [[] for _ in jobs]
+            list(pool.map(lambda jl: _run(jl[0], verbose, jl[1]), zip(jobs, logs)))
+        for l in logs:
+            log.extend(l)
     if force or _newer(LIB, objs):
         _run([NVCC, "-shared", "-o", LIB] + objs + ["-lquadmath"], verbose, log)
     with open(os.path.join(OBJ, "build.log"), "a") as f:
