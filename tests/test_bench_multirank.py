@@ -62,3 +62,30 @@ def test_reference_arm_runs_on_rank_zero_only():
     d = json.loads(lines[0])
     assert d["impl"] == "reference" and d["cpu_baseline"]["kind"] == "oracle" and d["gpu_launches"] == 0
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["value"] > 0 and d["unit"] == "GDOF-stage/s"
+
+
+def test_roofline_arithmetic_of_the_bench_line():
+    """rooflines(): algorithmic flops / bytes per launch over the measured kernel time against the two peaks; the
+    binding roof is the one with the larger fraction, the other goes to other_roof (SURVEY 8(d) figures)."""
+    import bench
+    assert bench.algorithmic_flop_per_dof_stage(3, 35, 15) == 380.0          # 2*3*35 + 2*4*15 + 50
+    assert bench.algorithmic_flop_per_dof_stage(2, 15, 5) == 140.0
+    assert bench.algorithmic_flop_per_dof_stage(3, 20, 10) == 250.0
+    dof = 196608 * 35 * 10
+    m = dict(dim=3, Np=35, Nfp=15, dof=dof, kern_ms=1.186, nprof=80, share=0.976, graph_timed=False)
+    r = bench.rooflines(m, 4, 0)
+    assert r["bound"] == "alu" and r["other_roof"]["bound"] == "hbm"
+    assert r["achieved"] == pytest.approx(dof * 380.0 / 1.186e-3 / 1e12)
+    assert r["frac"] == pytest.approx(r["achieved"] / (148 * 64 * 2 * 1.965e9 / 1e12))
+    assert r["other_roof"]["achieved"] == pytest.approx(dof * 38.0 / 1.186e-3 / 1e9)
+    assert r["traffic"] == pytest.approx(2.507e9) and r["algorithmic_bytes_per_launch"] == pytest.approx(dof * 38.0)
+    m2 = dict(dim=2, Np=15, Nfp=5, dof=60000 * 15 * 6, kern_ms=0.0699, nprof=60, share=None, graph_timed=True)
+    r2 = bench.rooflines(m2, 3, 0)
+    assert r2["bound"] == "hbm" and 0.4 < r2["frac"] < 0.5 and r2["other_roof"]["bound"] == "alu"
+    assert bench.rooflines(m2, 3, 1)["traffic"] is None                      # committed ncu traffic is the default kernel's
+
+
+def test_oracle_timing_helper_single_core():
+    import bench
+    v, cores, desc, ms = bench.time_oracle(1, 1, 0, cores=1)
+    assert cores == 1 and v > 0 and ms > 0 and "K=128" in desc
