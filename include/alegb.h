@@ -150,6 +150,39 @@ int alegb_get_cubature(alegb_ctx* ctx, int* degree, int* Nc, double* rst, double
  * ordered second pass).  A mesh without tagged faces gives zeros.  Errors: INVALID_ARG, NOT_READY, CUDA_ERROR. */
 int alegb_wall_forces(alegb_ctx* ctx, double t, const double* d_q, int tag, double* h_Fp, double* h_Fv, void* stream);
 
+/* The same integrals for callers that cannot allocate device memory at the point where they need the forces.
+ * Who that is: the forces are a per-time-step diagnostic (drag / lift histories, L308), so the call sits inside the
+ * time loop, and alegb_wall_forces cudaMallocs its partial-sum buffer the first time it runs -- that is, in the middle
+ * of the loop.  That does not work for (i) an application that, once the mesh is uploaded, gives all remaining HBM to
+ * its own pool (a framework's caching allocator, a solver's arena): cudaMalloc then returns out-of-memory although the
+ * pool has room; (ii) a time loop that keeps several streams busy and cannot take the device-wide stall that
+ * cudaMalloc / cudaFree bring with them; (iii) a caller that wants the result to stay on the device and the stream
+ * to keep running (alegb_wall_forces copies to the host and waits for the stream).
+ * This entry point calls no cudaMalloc, cudaFree or allocating library routine, copies nothing to the host and does
+ * not synchronise.  Its only scratch memory, the per-block partial sums of the first pass, is a fixed array inside the
+ * library image: ALEGB_WALL_FORCES_STATIC_MAX_BLOCKS x 6 doubles = 48 KiB on every GPU that loads libalegb.so, held
+ * until the process exits.
+ *   d_q      DEVICE [K][Nf][Np], read only
+ *   tag      boundary tag, 1..127
+ *   nblocks  thread blocks of the first pass = partial sums kept: 0 selects 296, the grid alegb_wall_forces uses, and
+ *            the result then equals that call's bit for bit; any other value 1..ALEGB_WALL_FORCES_STATIC_MAX_BLOCKS
+ *            changes only the order of the final sum (round-off).  Larger values do not fit the array and are
+ *            rejected with ALEGB_INVALID_ARG and a message naming the limit; nothing is launched.
+ *   d_F      DEVICE out [2 dim], caller-owned: F_p[0..dim) then F_v[0..dim); valid once `stream` has reached this
+ *            point.  A mesh without tagged faces gives zeros (a memset on `stream`).
+ * Geometry from the closed-form law at t, exactly as alegb_wall_forces (two more launches on `stream`).
+ * First call on each device: the library asks the runtime for the array's address on that device
+ * (cudaGetSymbolAddress, which may load the module there) and remembers it.  Make that first call during set-up,
+ * before any stream capture is begun in the process, and with no other work depending on its latency.
+ * Sharing: every call on a device -- from any context, any stream, any thread -- uses the one array.  Nothing in it
+ * needs to be zero beforehand (each launched block overwrites its own entry and only those entries are read), so
+ * calls that follow one another on a stream, or are ordered by events, are independent of each other.  Calls whose
+ * kernels may run concurrently on the same device are a data race on the partial sums: order them.
+ * Errors: INVALID_ARG (NULL pointer, tag, nblocks), NOT_READY, CUDA_ERROR. */
+#define ALEGB_WALL_FORCES_STATIC_MAX_BLOCKS 1024
+int alegb_wall_forces_static(alegb_ctx* ctx, double t, const double* d_q, int tag, int nblocks, double* d_F,
+                             void* stream);
+
 /* Select the coordinate mode.  RK: the library's current positions x_n are set to the law's positions at t_start
  * (kind USER: to the positions last given to alegb_set_motion_user); every alegb_step then advances them, so
  * consecutive calls must continue in time where the previous one ended.  alegb_step_debug reads x_n and leaves it

@@ -38,6 +38,7 @@ _SIGNATURES = {
     "alegb_set_geometry_overlap": (_c.c_int, [_P, _c.c_int]),
     "alegb_set_layer_fusion": (_c.c_int, [_P, _c.c_int]),
     "alegb_wall_forces": (_c.c_int, [_P, _c.c_double, _P, _c.c_int, _P, _P, _P]),
+    "alegb_wall_forces_static": (_c.c_int, [_P, _c.c_double, _P, _c.c_int, _c.c_int, _P, _P]),
     "alegb_get_cubature": (_c.c_int, [_P, _c.POINTER(_c.c_int), _c.POINTER(_c.c_int), _P, _P, _P, _P]),
     "alegb_get_positions": (_c.c_int, [_P, _P, _P]),
     "alegb_rhs": (_c.c_int, [_P, _c.c_double, _P, _P, _P]),
@@ -163,6 +164,12 @@ class Context:
         Fp, Fv = np.zeros(self.dim), np.zeros(self.dim)
         self._check(_lib.alegb_wall_forces(self._h, float(t), _dev(d_q), int(tag), Fp.ctypes.data, Fv.ctypes.data, _stream(stream)))
         return Fp, Fv
+
+    def alegb_wall_forces_static(self, t, d_q, d_F, tag=1, nblocks=0, stream=None):
+        """The wall forces for callers that cannot allocate where they need them (see include/alegb.h): d_F is the
+        caller's CUDA tensor of 2 dim doubles, filled with (F_p, F_v) on `stream`; the call allocates nothing, copies
+        nothing to the host and does not wait.  nblocks = 0 reproduces alegb_wall_forces bit for bit."""
+        self._check(_lib.alegb_wall_forces_static(self._h, float(t), _dev(d_q), int(tag), int(nblocks), _dev(d_F), _stream(stream)))
 
     def alegb_set_geometry_overlap(self, on):
         self._check(_lib.alegb_set_geometry_overlap(self._h, int(bool(on))))

@@ -790,6 +790,34 @@ int alegb_wall_forces(alegb_ctx* ctx, double t, const double* d_q, int tag, doub
   return ALEGB_OK;
 }
 
+// The no-allocation form of alegb_wall_forces (include/alegb.h): partial sums in the library's static device array
+// (kernels.cu), result left on the device, nothing allocated, nothing synchronised.
+int alegb_wall_forces_static(alegb_ctx* ctx, double t, const double* d_q, int tag, int nblocks, double* d_F,
+                             void* stream) {
+  int rc = check_ready(ctx);
+  if (rc != ALEGB_OK) return rc;
+  if (!d_q || !d_F) return fail(ctx, ALEGB_INVALID_ARG, "NULL pointer");
+  if (tag < 1 || tag > 127) return fail(ctx, ALEGB_INVALID_ARG, "tag must be a boundary tag (1..127)");
+  if (nblocks == 0) nblocks = 296;                      // the grid of alegb_wall_forces
+  if (nblocks < 0) return fail(ctx, ALEGB_INVALID_ARG, "nblocks must be 0 (default) or positive");
+  if (nblocks > ALEGB_WALL_FORCES_STATIC_MAX_BLOCKS)
+    return fail(ctx, ALEGB_INVALID_ARG,
+                "nblocks = " + std::to_string(nblocks) + " does not fit the static partial-sum array: the limit is "
+                "ALEGB_WALL_FORCES_STATIC_MAX_BLOCKS = " + std::to_string(ALEGB_WALL_FORCES_STATIC_MAX_BLOCKS));
+  const int dim = ctx->ref.dim;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (!ctx->d_EToB) {                                   // no tagged faces at all
+    CU(cudaMemsetAsync(d_F, 0, 2 * dim * sizeof(double), s));
+    return ALEGB_OK;
+  }
+  rc = update_geometry(ctx, t, s);
+  if (rc != ALEGB_OK) return rc;
+  CU(launch_wall_force_static(dim, ctx->K, ctx->d_EToB, tag, d_q, ctx->sg(), ctx->d_fmask, ctx->d_wface, ctx->ref.Np,
+                              ctx->ref.Nfp, ctx->RT, nblocks, d_F, s));
+  ctx->launches += 2;
+  return ALEGB_OK;
+}
+
 int alegb_set_coordinate_mode(alegb_ctx* ctx, int mode, double t_start) {
   if (!ctx) return ALEGB_INVALID_ARG;
   if (mode != ALEGB_COORDS_CLOSED_FORM && mode != ALEGB_COORDS_RK) return fail(ctx, ALEGB_INVALID_ARG, "unknown coordinate mode");

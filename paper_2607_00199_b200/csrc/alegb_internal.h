@@ -120,6 +120,11 @@ cudaError_t launch_vertex_rk(int dim, int64_t Nverts, const double* X0, const Mo
 cudaError_t launch_wall_force(int dim, int64_t K, const int8_t* EToB, int tag, const double* q, const double* sgeo,
                               const int32_t* fmask, const double* wface, int Np, int Nfp, double RT, double* partial,
                               int nblocks, double* out, cudaStream_t s);
+// the same with the partial sums in the library's static device array (no allocation; alegb_wall_forces_static);
+// the caller's device must be current; cudaErrorInvalidValue if nblocks is outside 1..ALEGB_WALL_FORCES_STATIC_MAX_BLOCKS
+cudaError_t launch_wall_force_static(int dim, int64_t K, const int8_t* EToB, int tag, const double* q,
+                                     const double* sgeo, const int32_t* fmask, const double* wface, int Np, int Nfp,
+                                     double RT, int nblocks, double* out, cudaStream_t s);
 // clock = {t0, dt, stage times[4]} on the device; _set starts a run of steps, the other advances to the next step
 cudaError_t launch_step_clock(double* clock, long long* counter, cudaStream_t s);
 cudaError_t launch_step_clock_set(double* clock, long long* counter, double t0, double dt, cudaStream_t s);

@@ -7,7 +7,9 @@
 //
 // The tensor-core (DMMA) stage kernel lives in stage_pipe.cu.
 #include <cstdio>
+#include <mutex>
 
+#include "../../include/alegb.h"
 #include "alegb_internal.h"
 #include "device_common.cuh"
 
@@ -275,6 +277,54 @@ cudaError_t launch_wall_force(int dim, int64_t K, const int8_t* EToB, int tag, c
   else wall_force_kernel<3><<<nblocks, 256, 0, s>>>(K, EToB, tag, q, sgeo, fmask, wface, Np, Nfp, RT, partial);
   wall_force_reduce_kernel<<<1, 32, 0, s>>>(partial, nblocks, 2 * dim, out);
   return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// The same two passes for callers that must not allocate (alegb_wall_forces_static, include/alegb.h).  The per-block
+// partial sums of the first pass live in an array that is part of the library image instead of in a cudaMalloc'd
+// buffer: kWallForceStaticBlocks x 6 doubles = 48 KiB, resident on every GPU that loads libalegb.so until the process
+// exits, whether or not the entry point is ever called.
+//
+// g_wall_force_partial is a DEVICE symbol.  In host code its name is only a handle for the runtime's symbol calls;
+// its value is not an address a kernel can use.  The address on the current device comes from cudaGetSymbolAddress,
+// and it differs from device to device, so it is looked up once per device and kept in a small host table.
+//
+// Nothing in the array has to start at zero: the first pass overwrites partial[b][0..2 dim) for every block b it
+// launches, including blocks that found no tagged face, and the second pass reads exactly those entries.  What a
+// previous call left behind is never read.  All calls on one device share the array, so two calls whose kernels can
+// run at the same time (different streams, no ordering between them) overwrite each other's partial sums.
+constexpr int kWallForceStaticBlocks = ALEGB_WALL_FORCES_STATIC_MAX_BLOCKS;
+constexpr int kWallForceStaticDevices = 64;
+static __device__ __align__(256) double g_wall_force_partial[kWallForceStaticBlocks * 6];
+static double* g_wall_force_partial_addr[kWallForceStaticDevices] = {};
+static std::mutex g_wall_force_partial_mutex;
+
+// Device address of g_wall_force_partial on the CURRENT device (the caller has made its device current).
+static cudaError_t wall_force_static_scratch(double** addr) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kWallForceStaticDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_wall_force_partial_mutex);
+  if (!g_wall_force_partial_addr[dev]) {
+    double* p = nullptr;
+    e = cudaGetSymbolAddress((void**)&p, g_wall_force_partial);   // loads the module on this device if need be
+    if (e != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    g_wall_force_partial_addr[dev] = p;
+  }
+  *addr = g_wall_force_partial_addr[dev];
+  return cudaSuccess;
+}
+
+cudaError_t launch_wall_force_static(int dim, int64_t K, const int8_t* EToB, int tag, const double* q,
+                                     const double* sgeo, const int32_t* fmask, const double* wface, int Np, int Nfp,
+                                     double RT, int nblocks, double* out, cudaStream_t s) {
+  if (nblocks < 1 || nblocks > kWallForceStaticBlocks) return cudaErrorInvalidValue;   // the ABI call checks first
+  double* partial = nullptr;
+  cudaError_t e = wall_force_static_scratch(&partial);
+  if (e != cudaSuccess) return e;
+  return launch_wall_force(dim, K, EToB, tag, q, sgeo, fmask, wface, Np, Nfp, RT, partial, nblocks, out, s);
 }
 
 // ------------------------------------------------------------------------------------------------------------------

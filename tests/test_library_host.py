@@ -168,7 +168,8 @@ def test_no_cpu_fallback():
                  lambda: ctx.alegb_profile_read(),
                  # the optional modes and the diagnostics have no host path either
                  lambda: ctx.alegb_set_relaxation(B.RELAX_CUBATURE), lambda: ctx.alegb_set_coordinate_mode(B.COORDS_RK, 0.0),
-                 lambda: ctx.alegb_get_positions(16, stream=0), lambda: ctx.alegb_wall_forces(0.0, 16, 1, stream=0)):
+                 lambda: ctx.alegb_get_positions(16, stream=0), lambda: ctx.alegb_wall_forces(0.0, 16, 1, stream=0),
+                 lambda: ctx.alegb_wall_forces_static(0.0, 16, 16, stream=0)):
         with pytest.raises(B.AlegbError) as e:
             call()
         assert e.value.status == B.CUDA_ERROR
