@@ -117,7 +117,9 @@ int alegb_set_params(alegb_ctx* ctx, double RT, double tau, const double* q_inf)
 int alegb_set_motion(alegb_ctx* ctx, int kind, const double* params, int nparams);
 /* kind USER: DEVICE arrays [Nverts*dim] of vertex positions and velocities, copied device-to-device on the
  * default stream and used for every subsequent evaluation (all four stages of every step: a velocity constant in
- * time) until the motion is set again.  Synchronises the default stream. */
+ * time) until the motion is set again.  Waits for the whole device first (a step still running on any stream,
+ * the library's side stream included, reads the buffers this call overwrites; it also makes arrays produced on
+ * another stream visible), copies on the default stream and synchronises it. */
 int alegb_set_motion_user(alegb_ctx* ctx, const double* d_xv, const double* d_vv);
 /* kind USER with data that change from stage to stage ("During each Runge-Kutta stage, we evaluate the
  * explicit, continuous velocity field v_G and subsequently update the spatial coordinates"; L391 fluid-structure
@@ -131,6 +133,8 @@ int alegb_set_motion_user(alegb_ctx* ctx, const double* d_xv, const double* d_vv
  *       x^(1) = x_n + dt/2 k_1,  x^(2) = x_n + dt/2 k_2,  x^(3) = x_n + dt k_3,  x_{n+1} = x_n + dt/6 (k_1+2k_2+2k_3+k_4),
  *     stage i of the fields sees x^(i) and k_{i+1}.
  * alegb_rhs, alegb_geometry and alegb_wall_forces (one evaluation, no stage) use entry 0.
+ * Synchronisation as alegb_set_motion_user: device-wide wait, copies, default stream synchronised -- calling it
+ * between single steps is safe whatever stream the steps run on, at the price of draining the device.
  * Errors: INVALID_ARG (d_vv4 NULL; d_xv4 NULL before any positions were supplied), NOT_READY, CUDA_ERROR. */
 int alegb_set_motion_user_stages(alegb_ctx* ctx, const double* d_xv4, const double* d_vv4);
 
@@ -250,6 +254,11 @@ int alegb_set_max_ctas(alegb_ctx* ctx, int max_ctas);
  * dynamic shared memory in bytes}.  ALEGB_UNSUPPORTED if there is no such kernel.  Needs no context and no device
  * (tests/test_pipe_protocol.py simulates the protocol with these numbers). */
 int alegb_pipe_config(int dim, int N, int* cfg);
+/* The same eight numbers for the instantiation that advances the absorbing layer inside the stage kernel (see
+ * alegb_set_layer_fusion): its slots carry dim more flux tiles, so it has one producer group and as many ring slots as
+ * shared memory allows, and a consumer warp releases a slot only after the directional contractions.
+ * ALEGB_UNSUPPORTED if (dim, N) has no such instantiation.  Needs no context and no device. */
+int alegb_pipe_config_layer(int dim, int N, int* cfg);
 /* Absorbing layer (a8): where the pipelined stage kernel runs and has an instantiation for it, the auxiliary fields of
  * the layer elements are advanced INSIDE the stage kernel (their D_a q, exterior traces and metrics are already on
  * chip there): the quads outside the layer run through the plain instantiation, the quads that touch the layer

@@ -62,6 +62,7 @@ _SIGNATURES = {
     "alegb_set_kernel": (_c.c_int, [_P, _c.c_int]),
     "alegb_set_max_ctas": (_c.c_int, [_P, _c.c_int]),
     "alegb_pipe_config": (_c.c_int, [_c.c_int, _c.c_int, _P]),
+    "alegb_pipe_config_layer": (_c.c_int, [_c.c_int, _c.c_int, _P]),
     "alegb_set_graph": (_c.c_int, [_P, _c.c_int]),
     "alegb_profile_enable": (_c.c_int, [_P, _c.c_int]),
     "alegb_profile_read": (_c.c_int, [_P, _c.POINTER(_c.c_int64), _c.POINTER(_c.c_double)]),
@@ -313,6 +314,15 @@ def alegb_pipe_config(dim, N):
     rc = _lib.alegb_pipe_config(int(dim), int(N), out)
     if rc != OK:
         raise AlegbError(rc, "alegb_pipe_config(dim=%d, N=%d)" % (dim, N))
+    return dict(zip(PIPE_CONFIG_FIELDS, (int(v) for v in out)))
+
+
+def alegb_pipe_config_layer(dim, N):
+    """The same for the instantiation with the absorbing layer fused in (alegb_set_layer_fusion)."""
+    out = (_c.c_int * 8)()
+    rc = _lib.alegb_pipe_config_layer(int(dim), int(N), out)
+    if rc != OK:
+        raise AlegbError(rc, "alegb_pipe_config_layer(dim=%d, N=%d)" % (dim, N))
     return dict(zip(PIPE_CONFIG_FIELDS, (int(v) for v in out)))
 
 

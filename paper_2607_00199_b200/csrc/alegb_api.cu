@@ -241,17 +241,27 @@ int timed_stage(alegb_ctx* ctx, const StageArgs& a_in, cudaStream_t s) {
   if (ctx->pipe_ok && (mode == 0 || mode == 2)) {
     if (a.layer.on) {
       // the quads outside the layer through the plain instantiation (deep ring, small slots), then the quads that
-      // touch it through the LAYER instantiation (a8 fused in)
-      StageArgs b = a;
-      b.layer.on = false; b.quad_list = ctx->d_quads_plain; b.nquads_list = ctx->nquads_plain;
-      CU(launch_stage_pipe(ctx->ref.dim, ctx->ref.N, b, ctx->ctas(), s));
+      // touch it through the LAYER instantiation (a8 fused in).  An empty list is not launched: the kernel reads a
+      // NULL quad_list as "every quad of the mesh", and a mesh whose every quad touches the layer has no plain list.
+      if (ctx->nquads_plain > 0) {
+        StageArgs b = a;
+        b.layer.on = false; b.quad_list = ctx->d_quads_plain; b.nquads_list = ctx->nquads_plain;
+        CU(launch_stage_pipe(ctx->ref.dim, ctx->ref.N, b, ctx->ctas(), s));
+        ctx->launches++;
+      }
+      if (ctx->nquads_layer > 0) {
+        a.quad_list = ctx->d_quads_layer; a.nquads_list = ctx->nquads_layer;
+        CU(launch_stage_pipe(ctx->ref.dim, ctx->ref.N, a, ctx->ctas(), s));
+        ctx->launches++;
+      }
+    } else {
+      CU(launch_stage_pipe(ctx->ref.dim, ctx->ref.N, a, ctx->ctas(), s));
       ctx->launches++;
-      a.quad_list = ctx->d_quads_layer; a.nquads_list = ctx->nquads_layer;
     }
-    CU(launch_stage_pipe(ctx->ref.dim, ctx->ref.N, a, ctx->ctas(), s));
+  } else {
+    CU(launch_stage(ctx->ref.dim, ctx->ref.N, a, ctx->ctas(), s));
+    ctx->launches++;
   }
-  else CU(launch_stage(ctx->ref.dim, ctx->ref.N, a, ctx->ctas(), s));
-  ctx->launches++;
   if (rec) {
     CU(cudaEventRecord(ctx->prof_events[ctx->prof_used + 1], s));
     ctx->prof_used += 2;
@@ -673,6 +683,11 @@ static int set_user_motion(alegb_ctx* ctx, const double* d_xv, const double* d_v
   const size_t n = (size_t)ctx->Nverts * ctx->ref.dim, bytes = n * sizeof(double);
   if (!ctx->d_user_xv) CU(dev_alloc(ctx, &ctx->d_user_xv, 4 * n));
   if (!ctx->d_user_vv) CU(dev_alloc(ctx, &ctx->d_user_vv, 4 * n));
+  // The buffers about to be overwritten are read by every a1 / a2 launch of a step, on the caller's stepping stream
+  // and on the library's side stream (the step graph keeps their addresses): wait for whatever is still in flight on
+  // ANY stream, non-blocking ones included, before the copies below go out on the default stream.  The same wait
+  // makes the caller's arrays visible if a kernel on another stream produced them.
+  CU(cudaDeviceSynchronize());
   for (int i = 0; i < 4; ++i) {
     if (d_xv) CU(cudaMemcpyAsync(ctx->d_user_xv + i * n, d_xv + i * stride, bytes, cudaMemcpyDeviceToDevice, 0));
     CU(cudaMemcpyAsync(ctx->d_user_vv + i * n, d_vv + i * stride, bytes, cudaMemcpyDeviceToDevice, 0));
@@ -1050,6 +1065,15 @@ int alegb_pipe_config(int dim, int N, int* cfg) {
   if (!cfg) return ALEGB_INVALID_ARG;
   PipeConfig c{};
   if (!stage_pipe_config(dim, N, c)) return ALEGB_UNSUPPORTED;
+  cfg[0] = c.producer_groups; cfg[1] = c.slots; cfg[2] = c.items_per_quad; cfg[3] = c.consumer_warps;
+  cfg[4] = c.warps_per_group; cfg[5] = c.producer_warps; cfg[6] = c.elements_per_quad; cfg[7] = c.smem_bytes;
+  return ALEGB_OK;
+}
+
+int alegb_pipe_config_layer(int dim, int N, int* cfg) {
+  if (!cfg) return ALEGB_INVALID_ARG;
+  PipeConfig c{};
+  if (!stage_pipe_config(dim, N, c, true)) return ALEGB_UNSUPPORTED;
   cfg[0] = c.producer_groups; cfg[1] = c.slots; cfg[2] = c.items_per_quad; cfg[3] = c.consumer_warps;
   cfg[4] = c.warps_per_group; cfg[5] = c.producer_warps; cfg[6] = c.elements_per_quad; cfg[7] = c.smem_bytes;
   return ALEGB_OK;

@@ -151,7 +151,7 @@ cudaError_t launch_pml_mma(int dim, int N, const PmlArgs& a, int num_sms, cudaSt
 cudaError_t configure_stage_pipe(int dim, int N);     // cudaErrorInvalidValue if (dim, N) has no such kernel
 cudaError_t launch_stage_pipe(int dim, int N, const StageArgs& a, int num_sms, cudaStream_t s);
 struct PipeConfig { int producer_groups, slots, items_per_quad, consumer_warps, warps_per_group, producer_warps, elements_per_quad, smem_bytes; };
-bool stage_pipe_config(int dim, int N, PipeConfig& c);   // false if (dim, N) has no such kernel
+bool stage_pipe_config(int dim, int N, PipeConfig& c, bool layer = false);   // false if (dim, N) has no such kernel; layer: the LAYER instantiation
 bool stage_pipe_layer_supported(int dim, int N);          // the instantiation with the absorbing layer fused in exists
 
 }  // namespace alegb

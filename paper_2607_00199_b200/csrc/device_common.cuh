@@ -88,37 +88,6 @@ __device__ __forceinline__ void hermite_apply(In in, double* y) {
   }
 }
 
-// The same matrices applied by COLUMN: the physical gradient gx[d] = d q_j / d x_d of ONE field j adds
-// c1 (A^_d)_kj gx[d] to V[k] (c2 = c1 sqrt2 for the sqrt2 entries).  The matrices are symmetric, so the rows fed by
-// column j of A^_d are the columns read by row j of hermite_apply.  j must be a compile-time constant after unrolling.
-template <int DIM>
-__device__ __forceinline__ void hermite_scatter(int j, const double* gx, double c1, double c2, double* V) {
-  auto add = [&](int k, int d, double cc) { V[k] = fma(cc, gx[d], V[k]); };
-  if constexpr (DIM == 2) {
-    switch (j) {
-      case 0: add(1, 0, c1); add(2, 1, c1); break;
-      case 1: add(0, 0, c1); add(4, 0, c2); add(3, 1, c1); break;
-      case 2: add(3, 0, c1); add(0, 1, c1); add(5, 1, c2); break;
-      case 3: add(2, 0, c1); add(1, 1, c1); break;
-      case 4: add(1, 0, c2); break;
-      default: add(2, 1, c2); break;
-    }
-  } else {
-    switch (j) {
-      case 0: add(1, 0, c1); add(2, 1, c1); add(3, 2, c1); break;
-      case 1: add(0, 0, c1); add(7, 0, c2); add(4, 1, c1); add(5, 2, c1); break;
-      case 2: add(4, 0, c1); add(0, 1, c1); add(8, 1, c2); add(6, 2, c1); break;
-      case 3: add(5, 0, c1); add(6, 1, c1); add(0, 2, c1); add(9, 2, c2); break;
-      case 4: add(2, 0, c1); add(1, 1, c1); break;
-      case 5: add(3, 0, c1); add(1, 2, c1); break;
-      case 6: add(3, 1, c1); add(2, 2, c1); break;
-      case 7: add(1, 0, c2); break;
-      case 8: add(2, 1, c2); break;
-      default: add(3, 2, c2); break;
-    }
-  }
-}
-
 template <int DIM>
 __device__ __forceinline__ void normal_apply(const double* nh, const double* x, double* y) {
   hermite_apply<DIM>([&](int d, int j) { return nh[d] * x[j]; }, y);

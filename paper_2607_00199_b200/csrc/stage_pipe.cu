@@ -668,27 +668,31 @@ bool stage_pipe_layer_supported(int dim, int N) {
 
 // The hand-over parameters of Cfg<DIM,N>, for tests/test_pipe_protocol.py (alegb_pipe_config): the simulation must
 // model the kernel that is compiled, not a re-typed copy of its constants.
-template <int DIM, int N>
+template <int DIM, int N, bool LAYER>
 static bool pipe_config_one(PipeConfig& c) {
-  using C = pipe::Cfg<DIM, N, false>;
+  using C = pipe::Cfg<DIM, N, LAYER>;
   if (!C::supported) return false;
   c.producer_groups = C::NG; c.slots = C::NS; c.items_per_quad = C::NB; c.consumer_warps = C::CW;
   c.warps_per_group = C::PG / 32; c.producer_warps = C::PW; c.elements_per_quad = C::EG; c.smem_bytes = (int)C::smem_bytes;
   return true;
 }
-bool stage_pipe_config(int dim, int N, PipeConfig& c) {
+template <bool LAYER>
+static bool pipe_config_any(int dim, int N, PipeConfig& c) {
   switch (dim * 10 + N) {
-    case 21: return pipe_config_one<2, 1>(c);
-    case 22: return pipe_config_one<2, 2>(c);
-    case 23: return pipe_config_one<2, 3>(c);
-    case 24: return pipe_config_one<2, 4>(c);
-    case 25: return pipe_config_one<2, 5>(c);
-    case 31: return pipe_config_one<3, 1>(c);
-    case 32: return pipe_config_one<3, 2>(c);
-    case 33: return pipe_config_one<3, 3>(c);
-    case 34: return pipe_config_one<3, 4>(c);
+    case 21: return pipe_config_one<2, 1, LAYER>(c);
+    case 22: return pipe_config_one<2, 2, LAYER>(c);
+    case 23: return pipe_config_one<2, 3, LAYER>(c);
+    case 24: return pipe_config_one<2, 4, LAYER>(c);
+    case 25: return pipe_config_one<2, 5, LAYER>(c);
+    case 31: return pipe_config_one<3, 1, LAYER>(c);
+    case 32: return pipe_config_one<3, 2, LAYER>(c);
+    case 33: return pipe_config_one<3, 3, LAYER>(c);
+    case 34: return pipe_config_one<3, 4, LAYER>(c);
     default: return false;
   }
+}
+bool stage_pipe_config(int dim, int N, PipeConfig& c, bool layer) {
+  return layer ? pipe_config_any<true>(dim, N, c) : pipe_config_any<false>(dim, N, c);
 }
 
 }  // namespace alegb

@@ -609,6 +609,55 @@ def test_wall_forces_match_oracle(name, refs, B):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("name,where", [("cfg3", "all"), ("cfg5_tiny", "all"), ("cfg5_tiny", "every_other_quad")])
+def test_layer_fusion_with_an_empty_or_interleaved_plain_list(name, where, refs, B):
+    """The fused path splits the quads into a plain and a layer launch.  With damping on every element (a whole-domain
+    sponge) the plain list is EMPTY and must not be launched at all (a NULL list means "every quad" to the kernel:
+    the mesh would be swept twice and stage 2's in-place accumulator doubled); with the layer on every other quad the
+    two lists interleave.  Stage states and auxiliary state of one step against the oracle, then five steps fused
+    against the separate layer kernel."""
+    ref, cfg = make_case(name, refs)
+    cfg = dict(cfg)
+    K, dim = cfg["EToV"].shape[0], cfg["dim"]
+    sig = np.array(cfg["pml_sigma"], dtype=np.float64, copy=True)
+    if where == "all":
+        sig += 0.5
+    else:
+        sig[:] = 0.0
+        sig[(np.arange(K) // 4) % 2 == 0] = (0.7, 0.0, 0.3)[:dim]
+    cfg["pml_sigma"] = sig
+    P = oracle_problem(cfg, ref)
+    q, dt = perturbed(cfg), cfg["dt"]
+    so, aux = sark.step_debug(P, q, 0.05, dt)
+    out = {}
+    for fused in (1, 0):
+        ctx = B.context_from_config(cfg)
+        ctx.alegb_set_layer_fusion(fused)
+        assert ctx.alegb_pml_count() == (K if where == "all" else ((np.arange(K) // 4) % 2 == 0).sum())
+        st = torch.empty((4,) + q.shape, dtype=torch.float64, device="cuda")
+        n0 = ctx.alegb_launch_count()
+        ctx.alegb_step_debug(dev(q), 0.05, dt, st)
+        nl = ctx.alegb_launch_count() - n0
+        da = torch.empty(aux.shape, dtype=torch.float64, device="cuda")
+        ctx.alegb_pml_get(da)
+        torch.cuda.synchronize()
+        for i in range(4):
+            assert rel_linf(st[i].cpu().numpy(), so[i]) <= TOL_STAGE, (fused, i)
+        assert np.abs(da.cpu().numpy() - aux).max() <= TOL_STAGE * max(np.abs(aux).max(), np.abs(q).max() * 1e-6)
+        dq = dev(q)
+        ctx.alegb_pml_reset()
+        ctx.alegb_step(dq, 0.0, dt, 5)
+        ctx.alegb_pml_get(da)
+        torch.cuda.synchronize()
+        out[fused] = (dq, da.clone(), nl)
+        ctx.close()
+    if where == "all":
+        assert out[1][2] < out[0][2]          # one stage launch per stage, not plain + layer
+    for x, y in zip(out[1][:2], out[0][:2]):
+        assert (x - y).abs().max().item() <= 1e-13 * max(y.abs().max().item(), 1e-300)
+
+
+@pytest.mark.gpu
 @pytest.mark.parametrize("name", ["cfg1", "cfg3", "cfg4"])
 def test_geometry_overlap_is_bit_identical(name, refs, B):
     """a1/a2 of stage i+1 beside the stage kernel of stage i (side stream, second geometry set): same bits as in-order

@@ -28,7 +28,7 @@ class Bar:
         return (self.phase & 1) != parity
 
 
-def simulate(NG, NS, NB, CW, WPG, NQ, seed, every_quad):
+def simulate(NG, NS, NB, CW, WPG, NQ, seed, every_quad, late_release=0):
     rng = random.Random(seed)
     full = [Bar(WPG) for _ in range(NS)]
     empty = [Bar(CW if every_quad else NB) for _ in range(NS)]
@@ -73,6 +73,10 @@ def simulate(NG, NS, NB, CW, WPG, NQ, seed, every_quad):
                     if content[slot] != q:
                         stale.append((cw, q, content[slot]))
                     yield
+                    for _ in range(late_release):          # LAYER: the directional contractions still read the
+                        if content[slot] != q:             # slot's flux tiles; it is released only after them
+                            stale.append((cw, q, content[slot]))
+                        yield
                 empty[slot].arrive()
         else:
             it = cw
@@ -100,16 +104,42 @@ def simulate(NG, NS, NB, CW, WPG, NQ, seed, every_quad):
     return False, stale
 
 
-def _cfg(dim, N):
+def _binding():
+    """The constants come from the built library; without it (a host that never ran the build) these tests skip
+    instead of failing at import."""
+    try:
+        from paper_2607_00199_b200 import binding
+    except (ImportError, OSError) as e:
+        pytest.skip("libalegb.so is not available: %s" % e)
+    return binding
+
+
+def _cfg(dim, N, layer=False):
     """(NG, NS, NB, CW, warps per group) of the kernel compiled for (dim, N), read from the library itself
-    (alegb_pipe_config reports Cfg<DIM,N> of csrc/stage_pipe.cu), so that the simulation cannot drift from the kernel."""
-    from paper_2607_00199_b200 import binding
-    c = binding.alegb_pipe_config(dim, N)
+    (alegb_pipe_config / alegb_pipe_config_layer report Cfg<DIM,N,LAYER> of csrc/stage_pipe.cu), so that the simulation
+    cannot drift from the kernel."""
+    binding = _binding()
+    c = (binding.alegb_pipe_config_layer if layer else binding.alegb_pipe_config)(dim, N)
     return c["producer_groups"], c["slots"], c["items_per_quad"], c["consumer_warps"], c["warps_per_group"]
 
 
 def test_library_reports_a_consistent_configuration():
-    from paper_2607_00199_b200 import binding
+    binding = _binding()
+    for dim, N in [(2, 1), (2, 4), (3, 1), (3, 3), (3, 4)]:
+        plain = binding.alegb_pipe_config(dim, N)
+        try:
+            layer = binding.alegb_pipe_config_layer(dim, N)
+        except binding.AlegbError as e:                          # 3-D N = 4: no ring of such slots fits shared memory
+            assert e.status == binding.UNSUPPORTED and (dim, N) == (3, 4)
+            continue
+        Np = (N + 1) * (N + 2) // 2 if dim == 2 else (N + 1) * (N + 2) * (N + 3) // 6
+        assert layer["items_per_quad"] == (Np + 7) // 8 <= layer["consumer_warps"]
+        assert layer["producer_groups"] * layer["warps_per_group"] == layer["producer_warps"]
+        assert layer["slots"] >= max(layer["producer_groups"], 2)
+        assert layer["smem_bytes"] <= 227 * 1024
+        assert layer["slots"] <= plain["slots"]                  # dim more flux tiles per slot
+        if dim == 3:
+            assert layer["producer_groups"] == 1                 # the four producer warps share one quad
     for dim, N in [(2, 1), (2, 4), (3, 1), (3, 3), (3, 4)]:
         c = binding.alegb_pipe_config(dim, N)
         Np = (N + 1) * (N + 2) // 2 if dim == 2 else (N + 1) * (N + 2) * (N + 3) // 6
@@ -126,6 +156,22 @@ def test_library_reports_a_consistent_configuration():
 def test_shipped_configurations_neither_deadlock_nor_read_stale_slots(dim, N):
     for seed in range(6):
         done, stale = simulate(*_cfg(dim, N), NQ=40, seed=seed, every_quad=True)
+        assert done and not stale
+
+
+@pytest.mark.parametrize("dim,N", [(2, 1), (2, 2), (2, 3), (2, 4), (2, 5), (3, 1), (3, 2), (3, 3), (3, 4)])
+def test_layer_configurations_neither_deadlock_nor_read_stale_slots(dim, N):
+    """The LAYER instantiation (the default stage kernel of a 3-D mesh with an absorbing layer): other producer
+    grouping and ring depth, and a consumer warp holds a slot through the directional contractions before it arrives
+    on `empty`."""
+    binding = _binding()
+    try:
+        cfg = _cfg(dim, N, layer=True)
+    except binding.AlegbError as e:
+        assert e.status == binding.UNSUPPORTED
+        pytest.skip("no LAYER instantiation for dim=%d N=%d (the separate layer kernel covers it)" % (dim, N))
+    for seed in range(6):
+        done, stale = simulate(*cfg, NQ=40, seed=seed, every_quad=True, late_release=1 + dim)
         assert done and not stale
 
 
