@@ -16,6 +16,8 @@ Metric: GDOF-stage updates/s = K_elements * Np * Nfields * 4 * steps / time.  On
   clocks       SM clock and throttle reasons polled through NVML in this process DURING the timed regions
   per_config   the other BASELINE.json workloads (1, 2, 3, 5): value, ms per step, stage-kernel time, both roofline
                fractions -- a driver-side record of every number DESIGN.md quotes
+  modes        the optional modes on the same box: config 4 with cubature-projected relaxation and with RK-integrated
+               coordinates, configs 3 / 5 with the absorbing layer fused into the stage kernel or separate
   cpu_baseline the oracle (oracle/, numpy, as it stands) on a bounded sample of the same workload, one independent
                replica per host core
   --impl reference   times the oracle alone (rank 0 only)
@@ -49,6 +51,11 @@ ALGO_BYTES_PER_DOF_STAGE = 38.0          # 152 B per DOF-step
 POINTWISE_FLOP_PER_DOF_STAGE = 50.0
 # dram__bytes_read.sum + dram__bytes_write.sum of the stage kernel per launch from committed `ncu --set full` captures
 # (mean over the stages of a step); configurations without a capture report no traffic figure.
+# The figures belong to the kernel they were captured from: NCU_CAPTURE_SHA256 is the sha256 over the stage kernel's
+# sources (kernel_sources_sha256) at the time of the capture.  With any other sources, or in a mode other than the
+# captured one (default kernel, collocated relaxation, closed-form coordinates, default layer fusion), the line
+# carries "traffic": null and says why in "traffic_source".
+NCU_CAPTURE_SHA256 = "8ed0e7f2d8713f72"   # round 2's sources (commit cbcb843)
 NCU_DRAM_BYTES_PER_LAUNCH = {
     4: (2.507e9, "profiles/r2_final.md"),
     # config 5: both stage launches of a stage (quads outside + inside the absorbing layer); includes a8's auxiliary
@@ -57,6 +64,16 @@ NCU_DRAM_BYTES_PER_LAUNCH = {
     3: (161.3e6, "profiles/r2_final.md"),
     2: (17.5e6, "profiles/r2_final.md")}
 DIM_N = {1: (2, 3), 2: (2, 4), 3: (2, 4), 4: (3, 4), 5: (3, 3)}
+
+
+def kernel_sources_sha256():
+    """sha256 (first 16 hex digits) over the sources the stage kernels are compiled from."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in ("stage_pipe.cu", "device_common.cuh"):
+        with open(os.path.join(ROOT, "paper_2607_00199_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
 
 
 def algorithmic_flop_per_dof_stage(dim, Np, Nfp):
@@ -204,8 +221,10 @@ def time_oracle(index, steps, warmup, cores=None):
     wall = max(r[0] for r in results)
     dof, K, name, N, Nf = results[0][1:6]
     assert all(r[6] for r in results)
-    desc = ("%s recipe shrunk to K=%d elements (N=%d, %d fields), %d SARK4 steps (%d stages), %d independent replicas "
-            "(one per host core, numpy single-threaded each)" % (name, K, N, Nf, steps, 4 * steps, cores))
+    desc = ("SAMPLE (K=%d), not the config: %s recipe shrunk to K=%d elements (N=%d, %d fields), %d SARK4 steps (%d "
+            "stages), %d independent replicas (one per host core, numpy single-threaded each); the value is the "
+            "aggregate of the replicas, no extrapolation to the full mesh"
+            % (K, name, K, N, Nf, steps, 4 * steps, cores))
     return cores * dof * 4 * steps / wall / 1e9, cores, desc, wall / max(steps, 1) * 1e3
 
 
@@ -261,6 +280,8 @@ def measure(index, args, B, torch, local_rank, world, barrier, sampler, repeats,
     ctx.alegb_set_kernel(args.kernel)
     if args.no_overlap:
         ctx.alegb_set_geometry_overlap(False)
+    if getattr(args, "layer_fusion", None) is not None:
+        ctx.alegb_set_layer_fusion(args.layer_fusion)
     if args.relax == "cubature":
         ctx.alegb_set_relaxation(B.RELAX_CUBATURE)
     if args.coords == "rk":
@@ -307,7 +328,7 @@ def measure(index, args, B, torch, local_rank, world, barrier, sampler, repeats,
                 finite=finite)
 
 
-def rooflines(m, index, kernel):
+def rooflines(m, index, kernel, default_modes=True):
     hbm_peak, hbm_src = measured_peaks()
     flop_per_dof = algorithmic_flop_per_dof_stage(m["dim"], m["Np"], m["Nfp"])
     tf = m["dof"] * flop_per_dof / (m["kern_ms"] * 1e-3) / 1e12
@@ -320,15 +341,30 @@ def rooflines(m, index, kernel):
            "peak_source": hbm_src, "algorithmic_bytes_per_dof_stage": ALGO_BYTES_PER_DOF_STAGE}
     first, other = (alu, hbm) if alu["frac"] >= hbm["frac"] else (hbm, alu)
     first = dict(first)
-    if kernel == 0 and index in NCU_DRAM_BYTES_PER_LAUNCH:
+    first["algorithmic_bytes_per_launch"] = m["dof"] * ALGO_BYTES_PER_DOF_STAGE
+    sha = kernel_sources_sha256()
+    if index not in NCU_DRAM_BYTES_PER_LAUNCH:
+        first["traffic_source"] = "no committed ncu capture for this workload"
+    elif kernel != 0 or not default_modes:
+        first["traffic_source"] = "the committed ncu capture is of the default kernel and modes, not of this run"
+    elif sha != NCU_CAPTURE_SHA256:
+        first["traffic_source"] = ("stale: the committed ncu capture (%s) is of kernel sources %s, this run's are %s"
+                                   % (NCU_DRAM_BYTES_PER_LAUNCH[index][1], NCU_CAPTURE_SHA256, sha))
+    else:
         first["traffic"], src = NCU_DRAM_BYTES_PER_LAUNCH[index]
-        first["traffic_unit"] = "bytes per launch (ncu dram read+write, %s)" % src
-        first["algorithmic_bytes_per_launch"] = m["dof"] * ALGO_BYTES_PER_DOF_STAGE
+        first["traffic_unit"] = "bytes per launch (ncu dram read+write)"
+        first["traffic_source"] = "committed ncu capture %s, kernel sources sha256 %s (matches this run)" % (src, sha)
     first.update({"kernel": "alegb stage kernel (fused volume+relaxation+surface+SARK update)",
                   "kernel_ms": m["kern_ms"], "kernel_launches_timed": m["nprof"], "kernel_share_of_step": m["share"],
                   "kernel_timed_in": "second pass, direct launches (timed regions replay the step graph)"
                   if m["graph_timed"] else "timed regions", "other_roof": other})
     return first
+
+
+def default_modes(args):
+    """True if the run is in the modes the committed ncu captures were taken in."""
+    return (args.relax == "collocation" and args.coords == "closed" and not args.no_overlap
+            and getattr(args, "layer_fusion", None) is None)
 
 
 def main():
@@ -423,7 +459,7 @@ def main():
                 st = 50 if idx in (1, 2) else (20 if idx == 3 else 5)
                 mm = measure(idx, args, B, torch, local_rank, 1, barrier, sampler, 3, st, 3)
                 el = float(np.median(mm["times"]))
-                rf = rooflines(mm, idx, args.kernel)
+                rf = rooflines(mm, idx, args.kernel, default_modes(args))
                 per_config[str(idx)] = {
                     "workload": workload_name(idx), "K": mm["K"], "dof": mm["dof"], "steps": st, "repeats": 3,
                     "value": job_throughput(mm["dof"], st, 1, el), "unit": UNIT, "ms_per_step": el / st,
@@ -437,6 +473,38 @@ def main():
                 torch.cuda.empty_cache()
             except Exception as e:      # a failed side measurement must not lose the headline line
                 per_config[str(idx)] = {"error": repr(e)[:300]}
+    # ---- the optional modes (NEXT-1, NEXT-2, a8 fused / separate): throughput and stage-kernel time, a few seconds each
+    modes = None
+    if not args.no_per_config and world == 1 and default_modes(args):
+        import copy
+        modes = {}
+        for name, idx, change in (("config4_relax_cubature", 4, dict(relax="cubature")),
+                                  ("config4_coords_rk", 4, dict(coords="rk")),
+                                  ("config3_layer_fused", 3, dict(layer_fusion=1)),
+                                  ("config3_layer_separate", 3, dict(layer_fusion=0)),
+                                  ("config5_layer_separate", 5, dict(layer_fusion=0))):
+            try:
+                a2 = copy.copy(args)
+                for k, v in change.items():
+                    setattr(a2, k, v)
+                st = 20 if idx == 3 else 5
+                mm = measure(idx, a2, B, torch, local_rank, 1, barrier, sampler, 3, st, 3)
+                el = float(np.median(mm["times"]))
+                rf = rooflines(mm, idx, args.kernel, False)
+                modes[name] = {
+                    "workload": workload_name(idx), "change": change, "steps": st, "repeats": 3,
+                    "value": job_throughput(mm["dof"], st, 1, el), "unit": UNIT, "ms_per_step": el / st,
+                    # per stage: everything the stage launches (cubature kernel + stage kernel(s)); the separate
+                    # layer kernel of layer_fusion = 0 is outside this bracket
+                    "stage_kernel_ms": mm["kern_ms"],
+                    "frac_fp64": (rf if rf["bound"] == "alu" else rf["other_roof"])["frac"],
+                    "frac_hbm": (rf if rf["bound"] == "hbm" else rf["other_roof"])["frac"],
+                    "gpu_launches_per_region": int(mm["launches"]), "state_finite": mm["finite"]}
+                mm["ctx"].close()
+                del mm
+                torch.cuda.empty_cache()
+            except Exception as e:
+                modes[name] = {"error": repr(e)[:300]}
     clocks = sampler.stop() if sampler else None
 
     if rank != 0:
@@ -444,7 +512,7 @@ def main():
             dist.destroy_process_group()
         return
 
-    roofline = rooflines(m, args.config, args.kernel)
+    roofline = rooflines(m, args.config, args.kernel, default_modes(args))
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
@@ -461,6 +529,8 @@ def main():
             "e2e": e2e, "gpu_launches": int(m["launches"]), "clocks": clocks, "roofline": roofline}
     if per_config is not None:
         line["per_config"] = per_config
+    if modes is not None:
+        line["modes"] = modes
     if not args.no_cpu_baseline:
         v, cores, desc, _ = time_oracle(args.config, 6 if args.config in (4, 5) else 20, 1)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,

@@ -78,7 +78,22 @@ def test_roofline_arithmetic_of_the_bench_line():
     assert r["achieved"] == pytest.approx(dof * 380.0 / 1.186e-3 / 1e12)
     assert r["frac"] == pytest.approx(r["achieved"] / (148 * 64 * 2 * 1.965e9 / 1e12))
     assert r["other_roof"]["achieved"] == pytest.approx(dof * 38.0 / 1.186e-3 / 1e9)
-    assert r["traffic"] == pytest.approx(2.507e9) and r["algorithmic_bytes_per_launch"] == pytest.approx(dof * 38.0)
+    assert r["algorithmic_bytes_per_launch"] == pytest.approx(dof * 38.0)
+    # the committed ncu traffic figure belongs to the sources it was captured from: reported only while they match
+    if bench.kernel_sources_sha256() == bench.NCU_CAPTURE_SHA256:
+        assert r["traffic"] == pytest.approx(bench.NCU_DRAM_BYTES_PER_LAUNCH[4][0]) and "matches" in r["traffic_source"]
+    else:
+        assert r["traffic"] is None and r["traffic_source"].startswith("stale")
+    saved = bench.NCU_CAPTURE_SHA256
+    try:
+        bench.NCU_CAPTURE_SHA256 = bench.kernel_sources_sha256()
+        assert bench.rooflines(m, 4, 0)["traffic"] == pytest.approx(bench.NCU_DRAM_BYTES_PER_LAUNCH[4][0])
+        assert bench.rooflines(m, 4, 0, default_modes=False)["traffic"] is None   # --relax cubature, --coords rk, ...
+        assert bench.rooflines(m, 1, 0)["traffic"] is None                        # no capture for config 1
+        bench.NCU_CAPTURE_SHA256 = "0" * 16
+        assert bench.rooflines(m, 4, 0)["traffic"] is None
+    finally:
+        bench.NCU_CAPTURE_SHA256 = saved
     m2 = dict(dim=2, Np=15, Nfp=5, dof=60000 * 15 * 6, kern_ms=0.0699, nprof=60, share=None, graph_timed=True)
     r2 = bench.rooflines(m2, 3, 0)
     assert r2["bound"] == "hbm" and 0.4 < r2["frac"] < 0.5 and r2["other_roof"]["bound"] == "alu"
@@ -88,4 +103,4 @@ def test_roofline_arithmetic_of_the_bench_line():
 def test_oracle_timing_helper_single_core():
     import bench
     v, cores, desc, ms = bench.time_oracle(1, 1, 0, cores=1)
-    assert cores == 1 and v > 0 and ms > 0 and "K=128" in desc
+    assert cores == 1 and v > 0 and ms > 0 and "K=128" in desc and desc.startswith("SAMPLE (K=128), not the config")
