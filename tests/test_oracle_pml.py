@@ -1,0 +1,179 @@
+"""Pins of the absorbing layer's DIRECTIONAL pieces, one direction at a time (oracle/rhs.py, reading R12; no GPU).
+
+R12:  d q~^d/dt = G^d - sigma_d q~^d,   G^d = -c A^_d d_d q + LIFT(Fscale(-1/2 n_d c A^_d [q] + 1/2 n_d^2 |A_n| [q])).
+tests/test_oracle_pins.py pins the SUM over d (it must be the linear operator) and the -sigma_d q~^d coupling; a
+d <-> d' mix-up, or a central piece mis-scaled in one direction and compensated in another, passes those.  Here:
+
+  * strong consistency, per direction: for the nodal interpolant of a smooth field that varies differently in every
+    coordinate and every field, G^d alone converges to -c A^_d d_d q at the DG rate of a derivative (N);
+  * the weak-derivative identity, per direction, EXACT to round-off for arbitrary discontinuous data: tested against
+    a continuous piecewise polynomial phi,
+        sum_e int_e phi G^d  =  + c sum_e int_e (d_d phi) (A^_d q),
+    because -c A^_d (d_d q + LIFT(Fscale 1/2 n_d [q])) is the distributional derivative of a broken polynomial
+    (each face gives int phi n_d [q], half to either side) and the penalty 1/2 n_d^2 |A_n| [q] is equal and opposite
+    on the two sides of a face.  This fixes the sign and the factor 1/2 of the central piece, and its direction;
+    the partition n_d^2 of the penalty is free (any partition of unity sums to the full upwind penalty) and only
+    its antisymmetry is fixed;
+  * each test carries its negative control: directions swapped, and the central piece with its sign flipped, fail
+    by orders of magnitude -- the pins discriminate.
+
+A^_x, A^_y, A^_z are written out by hand from the Hermite recurrence xi h_i = sqrt(i+1) h_{i+1} + sqrt(i) h_{i-1}
+(field order of reading R3), not taken from oracle/physics.py.
+"""
+import numpy as np
+import pytest
+
+from oracle import motion
+from oracle.rhs import Problem
+from workloads import configs, meshes
+
+S2 = np.sqrt(2.0)
+INF = float("inf")
+
+# (row, column, value): row = the moment whose equation it is, column = the moment whose d_d derivative enters
+HAND_A = {
+    2: [  # fields (00, 10, 01, 11, 20, 02)
+        [(0, 1, 1.0), (1, 0, 1.0), (1, 4, S2), (2, 3, 1.0), (3, 2, 1.0), (4, 1, S2)],                      # A^_x
+        [(0, 2, 1.0), (1, 3, 1.0), (2, 0, 1.0), (2, 5, S2), (3, 1, 1.0), (5, 2, S2)],                      # A^_y
+    ],
+    3: [  # fields (000; 100, 010, 001; 110, 101, 011; 200, 020, 002)
+        [(0, 1, 1.0), (1, 0, 1.0), (1, 7, S2), (2, 4, 1.0), (3, 5, 1.0), (4, 2, 1.0), (5, 3, 1.0), (7, 1, S2)],
+        [(0, 2, 1.0), (1, 4, 1.0), (2, 0, 1.0), (2, 8, S2), (3, 6, 1.0), (4, 1, 1.0), (6, 3, 1.0), (8, 2, S2)],
+        [(0, 3, 1.0), (1, 5, 1.0), (2, 6, 1.0), (3, 0, 1.0), (3, 9, S2), (5, 1, 1.0), (6, 2, 1.0), (9, 3, S2)],
+    ],
+}
+
+
+def hand_matrix(dim, d):
+    nf = 6 if dim == 2 else 10
+    A = np.zeros((nf, nf))
+    for i, j, v in HAND_A[dim][d]:
+        A[i, j] = v
+    assert np.array_equal(A, A.T)
+    return A
+
+
+def layer_everywhere(dim, N, n, ref, moving=True):
+    """Periodic [0, 2 pi]^dim, every element flagged as layer (sigma_d = 1), mesh deformed by the motion law so that
+    the metric terms differ from element to element; evaluated at t = 0.2."""
+    L = 2 * np.pi
+    if dim == 2:
+        X0, EToV, eq = meshes.periodic_square(n, 0.0, L)
+        kind, params = motion.SINES_PRODUCT, [0.25, 1.0, 1.0, 1.0, 0.3, 0.1]
+    else:
+        X0, EToV, eq = meshes.periodic_cube(n, 0.0, L)
+        kind, params = motion.SINES_CROSS, [0.1, 1.0, 1.0, 0.4]
+    if not moving:
+        kind, params = motion.NONE, None
+    sigma = np.ones((EToV.shape[0], dim))
+    P = Problem(dim, N, X0, EToV, eq, None, sigma, RT=1.7, tau=INF, motion_kind=kind, motion_params=params, ref=ref)
+    return P
+
+
+def node_x(P, ref, t):
+    return configs.node_coordinates(P.geometry(t)["xv"], P.EToV, ref.lam)      # [K, Np, dim]
+
+
+# amplitudes, integer wave vectors and phases per field, written by hand: every field varies in every coordinate, with
+# different derivatives in each (a d <-> d' mix-up changes every entry of the expected result)
+AMP = [0.30, -0.20, 0.15, 0.25, -0.10, 0.12, 0.18, -0.22, 0.08, 0.14]
+KAP = {2: [(1, 2), (2, 1), (1, 1), (2, 2), (1, 2), (2, 1)],
+       3: [(1, 1, 0), (0, 1, 1), (1, 0, 1), (1, 1, 1), (1, 1, 0), (0, 1, 1), (1, 0, 1), (1, 1, 1), (1, 1, 0), (0, 1, 1)]}
+PHI = [0.0, 0.4, 0.9, 1.3, 2.1, 2.6, 3.0, 3.7, 4.2, 5.1]
+
+
+def smooth_field(dim, x):
+    """q[K, Nf, Np] and its exact partial derivatives dq[d][K, Nf, Np]."""
+    nf = 6 if dim == 2 else 10
+    q = np.zeros((x.shape[0], nf, x.shape[1]))
+    dq = [np.zeros_like(q) for _ in range(dim)]
+    for k in range(nf):
+        arg = PHI[k] + sum(KAP[dim][k][d] * x[..., d] for d in range(dim))
+        q[:, k] = (1.0 if k == 0 else 0.0) + AMP[k] * np.sin(arg)
+        for d in range(dim):
+            dq[d][:, k] = AMP[k] * KAP[dim][k][d] * np.cos(arg)
+    return q, dq
+
+
+def rms(a):
+    return float(np.sqrt(np.mean(a ** 2)))
+
+
+@pytest.mark.parametrize("dim,N,ns", [(2, 3, (8, 16)), (3, 3, (4, 8))])
+def test_each_directional_piece_converges_to_its_own_derivative(dim, N, ns, refs):
+    ref = refs(dim, N)
+    t = 0.2
+    errs, wrong = [], []
+    for n in ns:
+        P = layer_everywhere(dim, N, n, ref)
+        assert len(P.pml_elems) == P.K
+        q, dq = smooth_field(dim, node_x(P, ref, t))
+        F, G = P.rhs(q, t)                                         # aux = 0: G[:, d] is the piece itself
+        exact = [-P.c * np.einsum("fg,kgi->kfi", hand_matrix(dim, d), dq[d]) for d in range(dim)]
+        errs.append([rms(G[:, d] - exact[d]) for d in range(dim)])
+        # negative control: the piece of ANOTHER direction against this direction's derivative
+        wrong.append([rms(G[:, (d + 1) % dim] - exact[d]) for d in range(dim)])
+        assert all(rms(e) > 0.1 for e in exact)
+    for d in range(dim):
+        rate = np.log2(errs[0][d] / errs[1][d])
+        assert rate > N - 0.3, (d, errs, rate)
+        assert errs[1][d] < 0.02, (d, errs)         # the exact pieces have rms 0.12 ... 0.36: a wrong factor leaves >= 0.05
+        assert wrong[1][d] > 0.15 and wrong[1][d] > 0.8 * wrong[0][d], (d, wrong)     # the swapped piece stalls
+
+
+def weak_sides(P, ref, t, q, G, phi, dim):
+    """lhs[d][k] = sum_e J_e phi_e^T M G^d_e[k];  rhs[d][k] = c sum_e J_e (d_d phi)_e^T M (A^_d q)_e[k]."""
+    g = P.geometry(t)
+    J, Ginv = g["J"], g["Ginv"]                                    # Ginv[K, a, d] = d xi_a / d x_d
+    dphi_ref = [np.einsum("ij,kj->ki", ref.D[a], phi) for a in range(dim)]
+    lhs, rhs = [], []
+    for d in range(dim):
+        dphi = sum(Ginv[:, a, d, None] * dphi_ref[a] for a in range(dim))
+        Aq = np.einsum("fg,kgi->kfi", hand_matrix(dim, d), q)
+        lhs.append(np.einsum("k,ki,ij,kfj->f", J, phi, ref.M, G[:, d]))
+        rhs.append(P.c * np.einsum("k,ki,ij,kfj->f", J, dphi, ref.M, Aq))
+    return np.array(lhs), np.array(rhs)
+
+
+@pytest.mark.parametrize("dim,N,n", [(2, 3, 4), (2, 4, 3), (3, 2, 3), (3, 3, 3)])
+def test_each_directional_piece_is_the_weak_derivative_of_broken_data(dim, N, n, refs):
+    ref = refs(dim, N)
+    t = 0.2
+    P = layer_everywhere(dim, N, n, ref)
+    nf = 6 if dim == 2 else 10
+    rng = np.random.default_rng(5)
+    q = rng.standard_normal((P.K, nf, ref.Np))                     # O(1) jumps on every face
+    q[:, 0] += 3.0
+    x = node_x(P, ref, t)
+    phi = 1.0 + 0.5 * np.sin(x[..., 0] + 0.3) * np.cos(2 * x[..., 1] - 0.2) * (np.sin(x[..., 2] + 1.0) if dim == 3 else 1.0)
+    # phi is single-valued at the shared face nodes, hence continuous: the identity needs nothing else of it
+    F, G = P.rhs(q, t)
+    lhs, rhs = weak_sides(P, ref, t, q, G, phi, dim)
+    scale = np.abs(rhs).max()
+    assert scale > 1.0
+    assert np.abs(lhs - rhs).max() < 1e-11 * scale, (lhs, rhs)
+
+    # ---- negative controls: the identity is violated at O(1) by the mistakes it is there to catch
+    # (i) directions mixed up: piece d' delivered as piece d
+    Gs = G[:, [(d + 1) % dim for d in range(dim)]]
+    lhs_s, _ = weak_sides(P, ref, t, q, Gs, phi, dim)
+    assert np.abs(lhs_s - rhs).max() > 0.05 * scale
+    # (ii) the central piece with the wrong sign (volume part recomputed here from D, the metric and the hand-written
+    #      matrices; what is left of G^d is its surface part)
+    g = P.geometry(t)
+    dref = [np.einsum("ij,kfj->kfi", ref.D[a], q) for a in range(dim)]
+    Gf = np.empty_like(G)
+    for d in range(dim):
+        grad_d = sum(g["Ginv"][:, a, d, None, None] * dref[a] for a in range(dim))
+        vol = -P.c * np.einsum("fg,kgi->kfi", hand_matrix(dim, d), grad_d)
+        Gf[:, d] = vol - (G[:, d] - vol)
+    lhs_f, _ = weak_sides(P, ref, t, q, Gf, phi, dim)
+    assert np.abs(lhs_f - rhs).max() > 0.05 * scale
+    # (iii) a central piece scaled by 1.5 in x and compensated in y so that the SUM over directions is unchanged
+    Gc = G.copy()
+    extra = 0.5 * (G[:, 0] - (Gf[:, 0] + G[:, 0]) / 2.0)           # half of the x surface part
+    Gc[:, 0] += extra
+    Gc[:, 1] -= extra
+    assert np.abs(Gc.sum(axis=1) - G.sum(axis=1)).max() < 1e-12 * np.abs(G).max()     # test_pml_invariants cannot see it
+    lhs_c, _ = weak_sides(P, ref, t, q, Gc, phi, dim)
+    assert np.abs(lhs_c - rhs).max() > 0.02 * scale
