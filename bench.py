@@ -55,14 +55,14 @@ POINTWISE_FLOP_PER_DOF_STAGE = 50.0
 # sources (kernel_sources_sha256) at the time of the capture.  With any other sources, or in a mode other than the
 # captured one (default kernel, collocated relaxation, closed-form coordinates, default layer fusion), the line
 # carries "traffic": null and says why in "traffic_source".
-NCU_CAPTURE_SHA256 = "8ed0e7f2d8713f72"   # round 2's sources (commit cbcb843)
+NCU_CAPTURE_SHA256 = "13631ba549af3491"   # sources of the round-3 captures (profiles/r3_final.md)
 NCU_DRAM_BYTES_PER_LAUNCH = {
-    4: (2.507e9, "profiles/r2_final.md"),
+    4: (2.506e9, "profiles/r3_final.md"),
     # config 5: both stage launches of a stage (quads outside + inside the absorbing layer); includes a8's auxiliary
     # arrays (up to 5 arrays x 3 directions x 8 B per layer DOF), which the 38 B per DOF-stage do not count
-    5: (21.94e9, "profiles/r2_final.md"),
-    3: (161.3e6, "profiles/r2_final.md"),
-    2: (17.5e6, "profiles/r2_final.md")}
+    5: (21.88e9, "profiles/r3_final.md"),
+    3: (160.9e6, "profiles/r3_final.md"),
+    2: (17.45e6, "profiles/r3_final.md")}
 DIM_N = {1: (2, 3), 2: (2, 4), 3: (2, 4), 4: (3, 4), 5: (3, 3)}
 
 

@@ -12,7 +12,9 @@ In the physical sign convention (reading R2) and with the collocated r
 Geometry, mesh velocity, volume and surface terms are all evaluated at the same time t (L154, GCL).
 
 Boundary states and the absorbing layer are NOT printed in the paper (boundary conditions are never stated;
-L5/L371 only name the PML): "parity unpinned by the paper".  They follow DESIGN.md readings R11 and R12:
+L5/L371 only name the PML): the paper offers no value to compare with.  They follow DESIGN.md readings R11 and R12
+and are pinned by invariants (tests/test_oracle_pins.py) and, for the layer's pieces one direction at a time, by
+consistency, the weak-derivative identity and a reflection test (tests/test_oracle_pml.py):
   wall (tag 1, moves with the mesh):  q1+ = q1-,  q_m+ = 2 q1- v_G,m / c - q_m- (momentum fields),  rest q+ = q-;
   far field (tag 2):                  q+ = q_inf;
   PML (elements with sigma_d > 0):    auxiliary fields qt^d, d = 1..dim, with

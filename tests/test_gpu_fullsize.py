@@ -225,18 +225,35 @@ def test_full_size_config5_sampled(refs, B):
     opos = np.searchsorted(patch[Psub.pml_elems], sl)
     assert len(sl) >= 24
     assert np.abs(Gg - G[opos]).max() <= TOL_F * (Fabs[where].max() + np.abs(G).max())
-    # stage states of one step on 10 of the samples (4 rings each, one patch), auxiliary state from zero
-    s10 = np.unique(np.concatenate([pick(wall, 3), pick(far, 3), pick(layer, 2), [0, K - 1]]))
+    # stage states of one step on >= 64 samples (4 rings each, one patch), auxiliary state from zero: wall, far field,
+    # layer elements with one / two / three damped directions, elements just outside the layer, random ones, the
+    # first and the last quad; and the auxiliary state after the step on the sampled layer elements
+    nlive = (sigma > 0).sum(axis=1)
+    one, two, three = (np.nonzero(nlive == k)[0] for k in (1, 2, 3))
+    assert len(one) > 100000 and len(two) > 10000 and len(three) > 1000
+    s64 = np.unique(np.concatenate([pick(wall, 12), pick(far, 12), pick(one, 12), pick(two, 12), pick(three, 8),
+                                    rng.integers(0, K, size=8), [0, 1, 2, 3, K - 4, K - 3, K - 2, K - 1]]))
+    assert len(s64) >= 64
     ctx.alegb_pml_reset()
     st = torch.empty((4,) + q.shape, dtype=torch.float64, device="cuda")
     ctx.alegb_step_debug(dq, t, dt, st)
+    da = torch.empty_like(daux)
+    ctx.alegb_pml_get(da)
     torch.cuda.synchronize()
-    sub, patch, where = submesh(cfg, conn["EToE"], s10, rings=4)
-    so, _ = sark.step_debug(oracle_problem(sub, ref), sub["q0"], t, dt)
-    idx = torch.from_numpy(s10).cuda()
+    sub, patch, where = submesh(cfg, conn["EToE"], s64, rings=4)
+    Psub = oracle_problem(sub, ref)
+    so, auxo = sark.step_debug(Psub, sub["q0"], t, dt)
+    idx = torch.from_numpy(s64).cuda()
     for i in range(4):
         got = st[i][idx].cpu().numpy()
         assert np.abs(got - so[i][where]).max() <= TOL_STAGE * np.abs(so[i]).max()
+    sl = s64[np.isin(s64, layer)]
+    assert len(sl) >= 32
+    got = da[torch.from_numpy(np.searchsorted(layer, sl)).cuda()].cpu().numpy()
+    want = auxo[np.searchsorted(patch[Psub.pml_elems], sl)]
+    # where sigma_d = 0 the auxiliary field never reaches q (it enters only as -sigma_d q~^d): compared where it can
+    live = (sigma[sl] > 0)[:, :, None, None]
+    assert np.abs((got - want) * live).max() <= TOL_STAGE * max(np.abs(auxo).max(), np.abs(q).max() * 1e-6)
     ctx.close()
 
 
