@@ -444,6 +444,19 @@ def main():
                "batched": {"value": job_throughput(dof, args.steps, world, el_b * 1e3), "unit": UNIT,
                            "steps_per_call": args.steps, "h2d_bytes_per_step": state_bytes / args.steps,
                            "d2h_bytes_per_step": state_bytes / args.steps}}
+    # fp64 ceiling measured on this device at the clocks of this run (alegb_measure_fp64_peak), for the roofline
+    fp64_measured = None
+    try:
+        if sampler:
+            sampler.begin()
+        dmma_tf, dfma_tf = ctx.alegb_measure_fp64_peak()
+        if sampler:
+            sampler.end()
+        fp64_measured = {"dmma_tflops": dmma_tf, "dfma_tflops": dfma_tf,
+                         "how": "alegb_measure_fp64_peak: register-resident DMMA (mma.sync.m8n8k4.f64) / DFMA chains, 16 "
+                                "warps per SM, best of 5 launches, CUDA events; clocks sampled during it (see clocks)"}
+    except Exception as e:
+        fp64_measured = {"error": repr(e)[:200]}
     ctx.close()
     del m["q"]
     torch.cuda.empty_cache()
@@ -513,6 +526,11 @@ def main():
         return
 
     roofline = rooflines(m, args.config, args.kernel, default_modes(args))
+    alu = roofline if roofline["bound"] == "alu" else roofline["other_roof"]
+    alu["peak_measured"] = fp64_measured
+    if fp64_measured and "dmma_tflops" in fp64_measured:
+        top = max(fp64_measured["dmma_tflops"], fp64_measured["dfma_tflops"])
+        alu["frac_of_measured_peak"] = alu["achieved"] / top if top > 0 else None
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",

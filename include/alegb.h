@@ -283,6 +283,12 @@ int alegb_set_graph(alegb_ctx* ctx, int on);
  * device and returns the number of bracketed launches and the sum of their durations in milliseconds. */
 int alegb_profile_enable(alegb_ctx* ctx, int on);
 int alegb_profile_read(alegb_ctx* ctx, int64_t* launches, double* total_ms);
+/* The fp64 ceiling of the context's device, measured: two register-resident microbenchmarks (chains of
+ * mma.sync.m8n8k4.f64 = DMMA, and of DFMA; 16 warps per SM, 8 independent accumulator sets each), best of 5 timed
+ * launches after a warm-up, CUDA events.  HOST out, TFLOP/s.  This is the denominator of the stage kernels' binding
+ * roofline (fp64-bound at N >= 3 in 3-D); bench.py reports it beside the figure derived from unit counts
+ * and the clock.  Takes about 50 ms, synchronises the device.  Errors: INVALID_ARG, CUDA_ERROR. */
+int alegb_measure_fp64_peak(alegb_ctx* ctx, double* dmma_tflops, double* dfma_tflops);
 /* Synchronous convenience entry for host buffers (HOST q [K][Nf][Np], updated in place): copies q to the device,
  * runs nsteps SARK4 steps, copies the result back.  Everything is enqueued on the LEGACY DEFAULT STREAM (stream 0),
  * which the call synchronises before it returns; the whole state crosses PCIe twice per call, so the cost per step

@@ -66,6 +66,7 @@ _SIGNATURES = {
     "alegb_set_graph": (_c.c_int, [_P, _c.c_int]),
     "alegb_profile_enable": (_c.c_int, [_P, _c.c_int]),
     "alegb_profile_read": (_c.c_int, [_P, _c.POINTER(_c.c_int64), _c.POINTER(_c.c_double)]),
+    "alegb_measure_fp64_peak": (_c.c_int, [_P, _c.POINTER(_c.c_double), _c.POINTER(_c.c_double)]),
 }
 for _name, (_res, _args) in _SIGNATURES.items():
     _fn = getattr(_lib, _name)          # AttributeError here = the library does not export a declared symbol
@@ -171,6 +172,12 @@ class Context:
         caller's CUDA tensor of 2 dim doubles, filled with (F_p, F_v) on `stream`; the call allocates nothing, copies
         nothing to the host and does not wait.  nblocks = 0 reproduces alegb_wall_forces bit for bit."""
         self._check(_lib.alegb_wall_forces_static(self._h, float(t), _dev(d_q), int(tag), int(nblocks), _dev(d_F), _stream(stream)))
+
+    def alegb_measure_fp64_peak(self):
+        """-> (DMMA TFLOP/s, DFMA TFLOP/s) measured on the context's device."""
+        a, b = _c.c_double(0.0), _c.c_double(0.0)
+        self._check(_lib.alegb_measure_fp64_peak(self._h, _c.byref(a), _c.byref(b)))
+        return a.value, b.value
 
     def alegb_set_geometry_overlap(self, on):
         self._check(_lib.alegb_set_geometry_overlap(self._h, int(bool(on))))

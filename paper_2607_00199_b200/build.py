@@ -21,7 +21,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 CXX_FLAGS = ["-O2", "-std=c++17", "-fPIC"]
 
-CU_SOURCES = ["kernels.cu", "stage_pipe.cu", "pml_mma.cu", "cubature.cu", "alegb_api.cu"]
+CU_SOURCES = ["kernels.cu", "stage_pipe.cu", "pml_mma.cu", "cubature.cu", "fp64_peak.cu", "alegb_api.cu"]
 CXX_SOURCES = ["host_ref.cpp"]
 HEADERS = ["alegb_internal.h", "device_common.cuh", "host_ref.h", os.path.join("..", "..", "include", "alegb.h")]
 

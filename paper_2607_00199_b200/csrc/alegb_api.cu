@@ -1122,6 +1122,16 @@ int alegb_profile_read(alegb_ctx* ctx, int64_t* launches, double* total_ms) {
   return ALEGB_OK;
 }
 
+int alegb_measure_fp64_peak(alegb_ctx* ctx, double* dmma_tflops, double* dfma_tflops) {
+  if (!ctx || !dmma_tflops || !dfma_tflops) return ALEGB_INVALID_ARG;
+  if (ctx->device < 0) return fail(ctx, ALEGB_CUDA_ERROR, "host-only context (no CUDA device)");
+  CU(cudaSetDevice(ctx->device));
+  CU(cudaDeviceSynchronize());
+  CU(measure_fp64_peak(ctx->num_sms, 5, dmma_tflops, dfma_tflops, 0));
+  ctx->launches += 12;
+  return ALEGB_OK;
+}
+
 int64_t alegb_workspace_bytes(const alegb_ctx* ctx) { return ctx ? ctx->workspace_bytes : 0; }
 const char* alegb_last_error(const alegb_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 int64_t alegb_launch_count(const alegb_ctx* ctx) { return ctx ? ctx->launches : 0; }

@@ -154,4 +154,7 @@ struct PipeConfig { int producer_groups, slots, items_per_quad, consumer_warps, 
 bool stage_pipe_config(int dim, int N, PipeConfig& c, bool layer = false);   // false if (dim, N) has no such kernel; layer: the LAYER instantiation
 bool stage_pipe_layer_supported(int dim, int N);          // the instantiation with the absorbing layer fused in exists
 
+// fp64 ceiling of the current device measured with register-resident DMMA / DFMA chains (fp64_peak.cu)
+cudaError_t measure_fp64_peak(int num_sms, int reps, double* dmma_tflops, double* dfma_tflops, cudaStream_t s);
+
 }  // namespace alegb

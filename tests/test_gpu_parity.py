@@ -580,6 +580,21 @@ def test_cubature_free_stream_on_gpu(refs, B):
     ctx.close()
 
 
+# ------------------------------------------------------------------ measurement: the fp64 ceiling bench.py reports
+@pytest.mark.gpu
+def test_measured_fp64_peak_is_plausible(refs, B):
+    """alegb_measure_fp64_peak: both microbenchmarks land near the figure derived from the unit counts
+    (148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2 TFLOP/s) -- well above half of it (the chains do run on every SM and
+    are not optimised away) and not above it by more than clock granularity allows."""
+    ref, cfg = make_case("cfg1", refs)
+    ctx = B.context_from_config(cfg)
+    dmma, dfma = ctx.alegb_measure_fp64_peak()
+    derived = 148 * 64 * 2 * 1.965e9 / 1e12
+    assert 0.5 * derived < dmma < 1.1 * derived, (dmma, dfma)
+    assert 0.5 * derived < dfma < 1.1 * derived, (dmma, dfma)
+    ctx.close()
+
+
 # ------------------------------------------------------------------ NEXT-3: wall-force integrals (L308, L369)
 @pytest.mark.gpu
 @pytest.mark.parametrize("name", ["cfg3", "cfg5", "cfg1"])

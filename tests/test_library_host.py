@@ -24,7 +24,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 def test_library_exports_every_declared_symbol():
     header = open(os.path.join(ROOT, "include", "alegb.h")).read()
-    declared = set(re.findall(r"\b(alegb_[a-z_]+)\s*\(", header))
+    declared = set(re.findall(r"\b(alegb_[a-z0-9_]+)\s*\(", header))
     assert len(declared) >= 20
     lib = ctypes.CDLL(B.LIB_PATH)
     for name in sorted(declared):
@@ -169,7 +169,7 @@ def test_no_cpu_fallback():
                  # the optional modes and the diagnostics have no host path either
                  lambda: ctx.alegb_set_relaxation(B.RELAX_CUBATURE), lambda: ctx.alegb_set_coordinate_mode(B.COORDS_RK, 0.0),
                  lambda: ctx.alegb_get_positions(16, stream=0), lambda: ctx.alegb_wall_forces(0.0, 16, 1, stream=0),
-                 lambda: ctx.alegb_wall_forces_static(0.0, 16, 16, stream=0)):
+                 lambda: ctx.alegb_wall_forces_static(0.0, 16, 16, stream=0), lambda: ctx.alegb_measure_fp64_peak()):
         with pytest.raises(B.AlegbError) as e:
             call()
         assert e.value.status == B.CUDA_ERROR
