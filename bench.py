@@ -446,15 +446,19 @@ def main():
                            "d2h_bytes_per_step": state_bytes / args.steps}}
     # fp64 ceiling measured on this device at the clocks of this run (alegb_measure_fp64_peak), for the roofline
     fp64_measured = None
+    # (clocks of the microbenchmark go into its own record: a pure DMMA loop runs into the power cap, and that reason
+    #  must not be attributed to the timed regions of the step)
     try:
-        if sampler:
-            sampler.begin()
+        peak_sampler = ClockSampler(local_rank) if rank == 0 else None
+        if peak_sampler:
+            peak_sampler.begin()
         dmma_tf, dfma_tf = ctx.alegb_measure_fp64_peak()
-        if sampler:
-            sampler.end()
+        if peak_sampler:
+            peak_sampler.end()
         fp64_measured = {"dmma_tflops": dmma_tf, "dfma_tflops": dfma_tf,
                          "how": "alegb_measure_fp64_peak: register-resident DMMA (mma.sync.m8n8k4.f64) / DFMA chains, 16 "
-                                "warps per SM, best of 5 launches, CUDA events; clocks sampled during it (see clocks)"}
+                                "warps per SM, best of 5 launches, CUDA events",
+                         "clocks": peak_sampler.stop() if peak_sampler else None}
     except Exception as e:
         fp64_measured = {"error": repr(e)[:200]}
     ctx.close()
